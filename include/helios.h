@@ -1,0 +1,138 @@
+/*
+ * helios.h -- C ABI of the B200-native batched Helios-r2 emission forward model.
+ *
+ * One call evaluates, for B candidate parameter vectors, the hot path of
+ * Kitzmann et al. 2020 (arXiv:1910.01070), Sect. 2.8:
+ * opacity interpolation -> absorption coefficient -> layer optical depths ->
+ * short-characteristics radiative transfer -> instrument profile -> binning ->
+ * log-likelihood.  Every step runs in hand-written sm_100a CUDA kernels; there
+ * is no CPU fallback: without a CUDA device helios_create() fails.
+ *
+ * Conventions
+ *   - plain C types only; every pointer argument says HOST or DEVICE.
+ *   - return value: 0 (HELIOS_OK) or a negative HELIOS_E* code; the message is
+ *     available from helios_last_error().  No C++ exception crosses the ABI.
+ *   - DEVICE-pointer entry points only ENQUEUE work on the context's CUDA stream
+ *     and return; they never synchronise the host.  The caller owns params and
+ *     output buffers and must keep them alive until the stream has passed the
+ *     enqueued work.  The *_host entry points copy, run and synchronise.
+ *   - the context owns its device copies of tables, observation and workspace;
+ *     host tables may be freed as soon as helios_load_opacity() returns.
+ *   - level index 0 = bottom of the atmosphere (highest pressure).
+ *   - units: cgs; wavenumbers in cm^-1; pressures in bar at the interface.
+ *   - not thread-safe per context; use one context per host thread / stream.
+ */
+#ifndef HELIOS_B200_H
+#define HELIOS_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct helios_ctx helios_ctx;   /* opaque */
+
+enum {
+    HELIOS_OK      =  0,
+    HELIOS_EINVAL  = -1,   /* bad argument (sizes, non-monotonic grids, bins outside the grid ...) */
+    HELIOS_ENOMEM  = -2,   /* device or host allocation failed                                     */
+    HELIOS_ECUDA   = -3,   /* a CUDA runtime call or kernel launch failed                          */
+    HELIOS_ESTATE  = -4    /* called before the tables / atmosphere / observation were set        */
+};
+
+#define HELIOS_PTRS_ON_DEVICE 1u   /* helios_load_opacity: sigma[s] / cia[c] are DEVICE pointers */
+
+/* helios_set_option keys */
+#define HELIOS_OPT_KERNEL      1   /* 0 = auto, 1 = direct (4-tap, global loads), 2 = slab (staged, large batch) */
+#define HELIOS_OPT_MODELS_PER_CTA 2/* slab kernel: models per CTA (0 = auto) */
+
+typedef struct helios_stats {
+    unsigned long long n_clamped;      /* (model, level) pairs whose (T, p) fell outside the table and were clamped */
+    unsigned long long n_nonfinite;    /* models rejected because a parameter was NaN/Inf                          */
+    unsigned long long n_models;       /* models evaluated since the last reset                                    */
+    unsigned long long n_launches;     /* kernels launched by this context since the last reset                    */
+} helios_stats;
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t
+ * (may be NULL = the legacy default stream); all work is enqueued on it.
+ * Fails with HELIOS_ECUDA if no CUDA device / sm_100 kernel image is usable. */
+int  helios_create (helios_ctx** out, int device, void* cuda_stream);
+void helios_destroy(helios_ctx* ctx);
+int  helios_set_stream(helios_ctx* ctx, void* cuda_stream);
+/* Message of the last failing call on this context (static storage inside ctx;
+ * ctx == NULL returns the message of the last failing helios_create). */
+const char* helios_last_error(const helios_ctx* ctx);
+int  helios_set_option(helios_ctx* ctx, int key, int value);
+
+/* Opacity tables.  Copies everything to HBM as fp32,
+ * nu-contiguous, rows padded to 128 B.
+ *   T_grid_K        HOST [nT]  strictly increasing, arbitrary spacing (nT >= 2)
+ *   log10p_grid_bar HOST [nP]  strictly increasing, arbitrary spacing (nP >= 2)
+ *   wavenumber grid nu_i = nu0_cm1 + i*dnu_cm1, i < nNu (uniform, dnu > 0)
+ *   sigma           HOST array of n_species pointers, each -> [nT][nP][nNu] fp32 cm^2
+ *                   (HOST data, or DEVICE data with HELIOS_PTRS_ON_DEVICE)
+ *   cia             HOST array of n_cia (0..2) pointers, each -> [nT][nNu] fp32,
+ *                   cm^-1 amagat^-2; pair 0 = H2-H2, pair 1 = H2-He (R4)
+ * Interpolation is bilinear in (T, log10 p) on sigma itself, linear in T for CIA;
+ * (T, p) outside the table is clamped to the edge and counted in helios_stats. */
+int helios_load_opacity(helios_ctx* ctx, int n_species,
+                        int nT, const double* T_grid_K,
+                        int nP, const double* log10p_grid_bar,
+                        int nNu, double nu0_cm1, double dnu_cm1,
+                        const float* const* sigma,
+                        int n_cia, const float* const* cia,
+                        unsigned flags);
+
+/* Atmosphere discretisation.
+ *   n_levels levels equidistant in log p from p_bottom_bar (level 0) to p_top_bar;
+ *   n_knots temperature nodes equidistant in log p (first-order elements);
+ *   n_angles Gauss-Legendre angles in mu in (0,1), 1..8;
+ *   mean_mol_weight in atomic mass units; he_to_h2 = He/H2 number ratio of the
+ *   background gas; flux_const = (R_star/d)^2 of Eq. 9.
+ * Requires helios_load_opacity() first (the pressure cells are resolved here). */
+int helios_set_atmosphere(helios_ctx* ctx, int n_levels, double p_bottom_bar, double p_top_bar,
+                          int n_knots, int n_angles, double mean_mol_weight, double he_to_h2,
+                          double flux_const);
+
+/* Observation (Eq. 17, 255, 267-270 Eq. 19).
+ *   bin_edges_cm1 HOST [n_bins+1] ascending, inside [nu_0, nu_{nNu-1}]
+ *   obs, obs_err  HOST [n_bins] (may both be NULL: spectra only, logL unavailable)
+ *   inst_sigma_cm1 HOST [nNu] Gaussian standard deviation at each grid point,
+ *                 or NULL = no instrument profile
+ * Builds, on the device, the banded operator that applies "convolve (cut at
+ * 5 sigma, renormalised) then bin-average" (R15, R17, R18). */
+int helios_set_observation(helios_ctx* ctx, int n_bins, const double* bin_edges_cm1,
+                           const double* obs, const double* obs_err,
+                           const double* inst_sigma_cm1);
+
+/* Pre-allocate workspace for batches up to max_batch (otherwise grown on demand,
+ * which synchronises the device once). */
+int helios_reserve(helios_ctx* ctx, int max_batch);
+
+/* The hot path.  params: DEVICE, row-major [B][P] fp64, P = 2 + n_knots + n_species:
+ *   log10 g (cgs), f (Eq. 9), T_knot[0..K-1] in K (bottom -> top), log10 VMR[0..S-1].
+ * spectra_out: DEVICE [B][n_bins] fp32 or NULL; logl_out: DEVICE [B] fp64 or NULL.
+ * A model with a non-finite parameter gets NaN spectra and logL = -inf; the
+ * other models are unaffected.  Enqueues only. */
+int helios_forward_batch(helios_ctx* ctx, int B, const double* params,
+                         float* spectra_out, double* logl_out);
+/* == helios_forward_batch(ctx, B, params, NULL, logl_out): spectra never written. */
+int helios_loglike_batch(helios_ctx* ctx, int B, const double* params, double* logl_out);
+/* Test hook: the flux of Eq. 9 on the native grid, before the instrument
+ * profile.  flux_out: DEVICE [B][nNu] fp32.  Needs no observation. */
+int helios_forward_highres(helios_ctx* ctx, int B, const double* params, float* flux_out);
+
+/* End-to-end variant: params, spectra_out (or NULL), logl_out (or NULL) are HOST
+ * buffers (pinned for full speed).  Copies params to the device, runs the hot
+ * path, copies the results back and synchronises the stream before returning. */
+int helios_forward_batch_host(helios_ctx* ctx, int B, const double* params_host,
+                              float* spectra_out_host, double* logl_out_host);
+
+/* Copies the counters (synchronises the stream); reset != 0 clears them. */
+int helios_get_stats(helios_ctx* ctx, helios_stats* out, int reset);
+/* HOST out: the angle set in use, mu[n_angles], w[n_angles]. */
+int helios_get_angles(const helios_ctx* ctx, double* mu_out, double* w_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HELIOS_B200_H */

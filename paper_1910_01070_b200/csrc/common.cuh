@@ -1,0 +1,83 @@
+// common.cuh -- constants, record layouts and small device helpers shared by the
+// kernels of libhelios_b200 (sm_100a only).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace helios {
+
+// CODATA 2018 (exact SI), cgs
+constexpr double kPlanckH   = 6.62607015e-27;     // erg s
+constexpr double kLightC    = 2.99792458e10;      // cm / s
+constexpr double kBoltzmann = 1.380649e-16;       // erg / K
+constexpr double kAtomicMass = 1.66053906660e-24; // g
+constexpr double kBarCgs    = 1.0e6;              // dyn / cm^2
+// 1 amagat: ideal-gas number density at 273.15 K, 101325 Pa
+constexpr double kAmagat    = 1.01325e6 / (kBoltzmann * 273.15);
+constexpr double kPi        = 3.14159265358979323846264338327950288;
+constexpr double kLog2e     = 1.44269504088896340735992468100189214;
+constexpr double kC1        = 2.0 * kPlanckH * kLightC * kLightC;   // 2 h c^2
+constexpr double kC2        = kPlanckH * kLightC / kBoltzmann;      // h c / k_B
+
+constexpr int kMaxAngles = 8;
+constexpr int kMaxCia = 2;
+
+// Per-(model, level) record written by the prep kernel for the DIRECT kernel, fp32:
+//   [0, 4S)        species tap weights  n x_s {(1-t)(1-u), (1-t)u, t(1-u), t u}
+//                  for table rows (iT,ip), (iT,ip+1), (iT+1,ip), (iT+1,ip+1)
+//   [4S, 4S+2C)    CIA tap weights      am^2 x_H2 x_c {(1-t), t}   rows iT, iT+1
+//   +0  planck_a   c2 log2(e) / T_l     (B_nu = c1 nu^3 E/(1-E), E = 2^(-planck_a nu))
+//   +1  hdz        dz_l / 2 of the layer between level l and l+1 (0 at the top level)
+//   +2  cell       iT*nP + ip           (int bits)
+//   +3  iT                               (int bits)
+__host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S + 2 * C + 4 + 3) & ~3; }
+
+// Slab kernel record, fp32 (p-blend is shared by all models, so 2 taps per row):
+//   [0, 2R)  pairs {a_r, b_r}: weights of the p-blended rows iT and iT+1, r < R = S + C
+//   +0 planck_a  +1 hdz  +2 iT (int bits)  +3 unused
+__host__ __device__ inline int slab_rec_floats(int R) { return (2 * R + 4 + 3) & ~3; }
+
+struct AngleSet {
+    int   n;
+    float c_exp[kMaxAngles];   // log2(e) / mu_k      : e^{-dtau/mu} = 2^(-dtau * c_exp)
+    float inv_mu[kMaxAngles];  // 1 / mu_k
+    float mu[kMaxAngles];
+    float wmu[kMaxAngles];     // w_k mu_k
+    float wmu_sum;             // sum_k w_k mu_k ( = 1/2 up to rounding)
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Short-characteristics update for one angle in deviation form.
+// With J = I - S(level) and dS = S_{l-1} - S_l, Eq. 4-6 read
+//   J_l = e^{-D} J_{l-1} + phi(D) dS,   phi(D) = (1 - e^{-D})/D,   D = dtau / mu  (Eq. 7)
+// (beta = 1 - phi, gamma = phi - e^{-D}).  phi is evaluated by its Taylor series for
+// D < kPhiSwitch, where (1 - e^{-D})/D cancels in fp32 (R10).
+constexpr float kPhiSwitch = 0.0625f;
+__device__ __forceinline__ float phi_series(float D) {
+    // 1 - D/2 + D^2/6 - D^3/24 + D^4/120 - D^5/720
+    float p = fmaf(D, -1.0f / 720.0f, 1.0f / 120.0f);
+    p = fmaf(D, p, -1.0f / 24.0f);
+    p = fmaf(D, p, 1.0f / 6.0f);
+    p = fmaf(D, p, -0.5f);
+    return fmaf(D, p, 1.0f);
+}
+__device__ __forceinline__ void sc_update(float& J, float dtau, float inv_dtau, float dS,
+                                          float c_exp, float inv_mu, float mu) {
+    float D = dtau * inv_mu;
+    float e = ex2_approx(-dtau * c_exp);
+    float phi_big = (1.0f - e) * (mu * inv_dtau);
+    float phi = (D < kPhiSwitch) ? phi_series(D) : phi_big;
+    J = fmaf(e, J, phi * dS);
+}
+
+}  // namespace helios

@@ -1,0 +1,551 @@
+// helios_api.cu -- C ABI of libhelios_b200 (include/helios.h): context, table
+// upload, atmosphere / observation setup, kernel launches.  sm_100a only.
+#include <math_constants.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/helios.h"
+#include "common.cuh"
+#include "obs.cuh"
+#include "prep.cuh"
+#include "rt_direct.cuh"
+#include "rt_slab.cuh"
+
+using namespace helios;
+
+struct helios_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    int num_sms = 148;
+
+    // ---- opacity tables
+    bool have_tables = false;
+    int S = 0, C = 0, nT = 0, nP = 0, nNu = 0;
+    long long stride = 0;               // padded row length, floats
+    double nu0 = 0, dnu = 0;
+    std::vector<double> T_grid, lp_grid;
+    float* d_sigma = nullptr;           // [S][nT][nP][stride]
+    float* d_cia = nullptr;             // [C][nT][stride]
+    double* d_Tgrid = nullptr;
+
+    // ---- atmosphere
+    bool have_atmo = false;
+    int L = 0, K = 0, A = 0;
+    double p_bot = 0, p_top = 0, mmw = 0, he_to_h2 = 0, flux_const = 1;
+    std::vector<double> mu, w;
+    AngleSet ang{};
+    double* d_lvl_p = nullptr; int* d_lvl_knot = nullptr; double* d_lvl_xi = nullptr;
+    int* d_lvl_ip = nullptr; double* d_lvl_u = nullptr; int* d_lvl_pclamp = nullptr;
+    double* d_lvl_lnratio = nullptr;
+    float* d_lvl_uf = nullptr;          // [L] fp32 pressure weight (slab kernel)
+    std::vector<int> lvl_ip;
+
+    // ---- observation
+    bool have_obs = false, have_data = false;
+    int J = 0;
+    double logl_const = 0;
+    double* d_edges = nullptr; double* d_obs = nullptr; double* d_inv2var = nullptr;
+    int* d_row_ptr = nullptr; int* d_row_lo = nullptr; float* d_W = nullptr;
+
+    // ---- workspace (grown on demand)
+    int cap_B = 0;
+    float* d_rec = nullptr; size_t rec_bytes = 0;
+    float* d_flux = nullptr; long long flux_stride = 0;
+    float* d_scale = nullptr; int* d_flag = nullptr;
+    unsigned long long* d_counters = nullptr;    // [2]
+    double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
+
+    // ---- options / statistics
+    int opt_kernel = 0, opt_models_per_cta = 0;
+    unsigned long long n_models = 0, n_launches = 0;
+};
+
+static std::string g_create_error;
+
+static int fail(helios_ctx* c, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf; else g_create_error = buf;
+    return code;
+}
+
+#define CU_TRY(c, call)                                                                      \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? HELIOS_ENOMEM : HELIOS_ECUDA, \
+                        "%s failed: %s", #call, cudaGetErrorString(e_));                     \
+    } while (0)
+
+template <class T>
+static void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
+
+template <class T>
+static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
+    dfree(dst);
+    cudaError_t e = cudaMalloc(&dst, sizeof(T) * (src.empty() ? 1 : src.size()));
+    if (e != cudaSuccess) return e;
+    if (!src.empty()) e = cudaMemcpyAsync(dst, src.data(), sizeof(T) * src.size(), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return e;
+    return cudaStreamSynchronize(s);     // src may be a temporary
+}
+
+static void free_all(helios_ctx* c) {
+    dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid);
+    dfree(c->d_lvl_p); dfree(c->d_lvl_knot); dfree(c->d_lvl_xi); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
+    dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio); dfree(c->d_lvl_uf);
+    dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
+    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_counters);
+    dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
+}
+
+extern "C" {
+
+int helios_create(helios_ctx** out, int device, void* cuda_stream) {
+    if (!out) return fail(nullptr, HELIOS_EINVAL, "helios_create: out is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return fail(nullptr, HELIOS_ECUDA, "helios_create: no CUDA device (%s); this library has no CPU fallback",
+                    e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+    if (device < 0 || device >= ndev) return fail(nullptr, HELIOS_EINVAL, "helios_create: device %d of %d", device, ndev);
+    e = cudaSetDevice(device);
+    if (e != cudaSuccess) return fail(nullptr, HELIOS_ECUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, k_prep);
+    if (e != cudaSuccess)
+        return fail(nullptr, HELIOS_ECUDA, "helios_create: no usable sm_100a kernel image on device %d (%s)", device,
+                    cudaGetErrorString(e));
+    helios_ctx* c = new (std::nothrow) helios_ctx();
+    if (!c) return fail(nullptr, HELIOS_ENOMEM, "helios_create: out of host memory");
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    e = cudaMalloc(&c->d_counters, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, 2 * sizeof(unsigned long long));
+    if (e != cudaSuccess) { delete c; return fail(nullptr, HELIOS_ECUDA, "helios_create: %s", cudaGetErrorString(e)); }
+    *out = c;
+    return HELIOS_OK;
+}
+
+void helios_destroy(helios_ctx* c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    free_all(c);
+    delete c;
+}
+
+int helios_set_stream(helios_ctx* c, void* s) {
+    if (!c) return HELIOS_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return HELIOS_OK;
+}
+
+const char* helios_last_error(const helios_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int helios_set_option(helios_ctx* c, int key, int value) {
+    if (!c) return HELIOS_EINVAL;
+    switch (key) {
+        case HELIOS_OPT_KERNEL:
+            if (value < 0 || value > 2) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1 or 2");
+            c->opt_kernel = value; return HELIOS_OK;
+        case HELIOS_OPT_MODELS_PER_CTA:
+            if (value < 0) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be >= 0");
+            c->opt_models_per_cta = value; return HELIOS_OK;
+        default: return fail(c, HELIOS_EINVAL, "unknown option %d", key);
+    }
+}
+
+int helios_load_opacity(helios_ctx* c, int S, int nT, const double* T_grid, int nP, const double* lp_grid,
+                        int nNu, double nu0, double dnu, const float* const* sigma, int C,
+                        const float* const* cia, unsigned flags) {
+    if (!c) return HELIOS_EINVAL;
+    if (S < 0 || S > 64 || C < 0 || C > kMaxCia || S + C < 1) return fail(c, HELIOS_EINVAL, "load_opacity: n_species %d, n_cia %d", S, C);
+    if (nT < 2 || nP < 2 || nNu < 2 || !(dnu > 0) || !T_grid || !lp_grid) return fail(c, HELIOS_EINVAL, "load_opacity: bad grid sizes");
+    for (int i = 1; i < nT; ++i) if (!(T_grid[i] > T_grid[i - 1])) return fail(c, HELIOS_EINVAL, "load_opacity: T grid not strictly increasing");
+    for (int i = 1; i < nP; ++i) if (!(lp_grid[i] > lp_grid[i - 1])) return fail(c, HELIOS_EINVAL, "load_opacity: log10 p grid not strictly increasing");
+    if ((S > 0 && !sigma) || (C > 0 && !cia)) return fail(c, HELIOS_EINVAL, "load_opacity: NULL table pointer array");
+    for (int s = 0; s < S; ++s) if (!sigma[s]) return fail(c, HELIOS_EINVAL, "load_opacity: sigma[%d] is NULL", s);
+    for (int k = 0; k < C; ++k) if (!cia[k]) return fail(c, HELIOS_EINVAL, "load_opacity: cia[%d] is NULL", k);
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_tables = c->have_atmo = c->have_obs = c->have_data = false;
+    dfree(c->d_sigma); dfree(c->d_cia);
+    c->S = S; c->C = C; c->nT = nT; c->nP = nP; c->nNu = nNu; c->nu0 = nu0; c->dnu = dnu;
+    c->stride = ((long long)nNu + 31) / 32 * 32;
+    c->T_grid.assign(T_grid, T_grid + nT);
+    c->lp_grid.assign(lp_grid, lp_grid + nP);
+    const cudaMemcpyKind kind = (flags & HELIOS_PTRS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    const size_t rows_s = (size_t)nT * nP;
+    if (S > 0) {
+        CU_TRY(c, cudaMalloc(&c->d_sigma, sizeof(float) * (size_t)S * rows_s * c->stride));
+        CU_TRY(c, cudaMemsetAsync(c->d_sigma, 0, sizeof(float) * (size_t)S * rows_s * c->stride, c->stream));
+        for (int s = 0; s < S; ++s)
+            CU_TRY(c, cudaMemcpy2DAsync(c->d_sigma + (size_t)s * rows_s * c->stride, sizeof(float) * c->stride, sigma[s],
+                                        sizeof(float) * nNu, sizeof(float) * nNu, rows_s, kind, c->stream));
+    }
+    if (C > 0) {
+        CU_TRY(c, cudaMalloc(&c->d_cia, sizeof(float) * (size_t)C * nT * c->stride));
+        CU_TRY(c, cudaMemsetAsync(c->d_cia, 0, sizeof(float) * (size_t)C * nT * c->stride, c->stream));
+        for (int k = 0; k < C; ++k)
+            CU_TRY(c, cudaMemcpy2DAsync(c->d_cia + (size_t)k * nT * c->stride, sizeof(float) * c->stride, cia[k],
+                                        sizeof(float) * nNu, sizeof(float) * nNu, nT, kind, c->stream));
+    }
+    CU_TRY(c, upload(c->d_Tgrid, c->T_grid, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_tables = true;
+    c->cap_B = 0;    // record size depends on S, C
+    return HELIOS_OK;
+}
+
+// n-point Gauss-Legendre rule on [-1, 1]: roots of P_n by Newton's method.
+static void gauss_legendre(int n, std::vector<double>& x, std::vector<double>& W) {
+    x.resize(n); W.resize(n);
+    for (int i = 0; i < (n + 1) / 2; ++i) {
+        double z = std::cos(kPi * (i + 0.75) / (n + 0.5)), pp = 1.0;
+        for (int it = 0; it < 64; ++it) {
+            double pa = 1.0, pb = 0.0;
+            for (int j = 0; j < n; ++j) {
+                double pc = pb; pb = pa;
+                pa = ((2.0 * j + 1.0) * z * pb - j * pc) / (j + 1.0);
+            }
+            pp = n * (z * pa - pb) / (z * z - 1.0);
+            double dz = pa / pp;
+            z -= dz;
+            if (std::fabs(dz) < 1e-15) break;
+        }
+        double pa = 1.0, pb = 0.0;
+        for (int j = 0; j < n; ++j) { double pc = pb; pb = pa; pa = ((2.0 * j + 1.0) * z * pb - j * pc) / (j + 1.0); }
+        pp = n * (z * pa - pb) / (z * z - 1.0);
+        x[i] = -z; x[n - 1 - i] = z;
+        W[i] = W[n - 1 - i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+}
+
+static void axis_cell(const std::vector<double>& grid, double v, int& i, double& w, int& clamped) {
+    const int n = (int)grid.size();
+    i = 0;
+    while (i < n - 2 && grid[i + 1] <= v) ++i;
+    w = (v - grid[i]) / (grid[i + 1] - grid[i]);
+    clamped = 0;
+    if (w < 0.0) { w = 0.0; clamped = 1; }
+    if (w > 1.0) { w = 1.0; clamped = 1; }
+}
+
+int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int K, int A, double mmw,
+                          double he_to_h2, double flux_const) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_tables) return fail(c, HELIOS_ESTATE, "set_atmosphere: call helios_load_opacity first");
+    if (L < 2 || L > 4096) return fail(c, HELIOS_EINVAL, "set_atmosphere: n_levels %d (2..4096)", L);
+    if (!(p_bot > p_top) || !(p_top > 0)) return fail(c, HELIOS_EINVAL, "set_atmosphere: need p_bottom > p_top > 0");
+    if (K < 1 || K > 64) return fail(c, HELIOS_EINVAL, "set_atmosphere: n_knots %d (1..64)", K);
+    if (A < 1 || A > kMaxAngles) return fail(c, HELIOS_EINVAL, "set_atmosphere: n_angles %d (1..%d)", A, kMaxAngles);
+    if (!(mmw > 0) || !(he_to_h2 >= 0) || !std::isfinite(flux_const)) return fail(c, HELIOS_EINVAL, "set_atmosphere: bad mmw / he_to_h2 / flux_const");
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_atmo = false;
+    c->L = L; c->K = K; c->A = A; c->p_bot = p_bot; c->p_top = p_top; c->mmw = mmw; c->he_to_h2 = he_to_h2;
+    c->flux_const = flux_const;
+
+    std::vector<double> p(L), xi(L), u(L), lnr(L, 0.0);
+    std::vector<int> knot(L), ip(L), pcl(L);
+    std::vector<float> uf(L);
+    const double x_bot = std::log10(p_bot), x_top = std::log10(p_top);
+    for (int l = 0; l < L; ++l) {
+        p[l] = p_bot * std::pow(p_top / p_bot, (double)l / (double)(L - 1));   // equidistant in log p
+        const double x = std::log10(p[l]);
+        double s = (K > 1) ? (x - x_bot) / (x_top - x_bot) * (K - 1) : 0.0;
+        int k = (int)std::floor(s);
+        if (k < 0) k = 0;
+        if (k > K - 2) k = K - 2 < 0 ? 0 : K - 2;
+        knot[l] = k; xi[l] = s - k;
+        axis_cell(c->lp_grid, x, ip[l], u[l], pcl[l]);
+        uf[l] = (float)u[l];
+    }
+    for (int l = 0; l + 1 < L; ++l) lnr[l] = std::log(p[l] / p[l + 1]);
+    c->lvl_ip = ip;
+    CU_TRY(c, upload(c->d_lvl_p, p, c->stream));
+    CU_TRY(c, upload(c->d_lvl_knot, knot, c->stream));
+    CU_TRY(c, upload(c->d_lvl_xi, xi, c->stream));
+    CU_TRY(c, upload(c->d_lvl_ip, ip, c->stream));
+    CU_TRY(c, upload(c->d_lvl_u, u, c->stream));
+    CU_TRY(c, upload(c->d_lvl_pclamp, pcl, c->stream));
+    CU_TRY(c, upload(c->d_lvl_lnratio, lnr, c->stream));
+    CU_TRY(c, upload(c->d_lvl_uf, uf, c->stream));
+
+    std::vector<double> x, W;
+    gauss_legendre(A, x, W);
+    c->mu.resize(A); c->w.resize(A);
+    AngleSet& g = c->ang;
+    std::memset(&g, 0, sizeof g);
+    g.n = A;
+    double wmu_sum = 0.0;
+    for (int k = 0; k < A; ++k) {
+        c->mu[k] = 0.5 * (x[k] + 1.0);
+        c->w[k] = 0.5 * W[k];
+        g.mu[k] = (float)c->mu[k];
+        g.inv_mu[k] = (float)(1.0 / c->mu[k]);
+        g.c_exp[k] = (float)(kLog2e / c->mu[k]);
+        g.wmu[k] = (float)(c->w[k] * c->mu[k]);
+        wmu_sum += c->w[k] * c->mu[k];
+    }
+    g.wmu_sum = (float)wmu_sum;
+    c->have_atmo = true;
+    c->cap_B = 0;
+    return HELIOS_OK;
+}
+
+int helios_get_angles(const helios_ctx* c, double* mu, double* w) {
+    if (!c || !c->have_atmo || !mu || !w) return HELIOS_EINVAL;
+    for (int k = 0; k < c->A; ++k) { mu[k] = c->mu[k]; w[k] = c->w[k]; }
+    return HELIOS_OK;
+}
+
+int helios_set_observation(helios_ctx* c, int J, const double* edges, const double* obs, const double* err,
+                           const double* inst_sigma) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_tables) return fail(c, HELIOS_ESTATE, "set_observation: call helios_load_opacity first");
+    if (J < 1 || !edges) return fail(c, HELIOS_EINVAL, "set_observation: n_bins %d", J);
+    if ((obs == nullptr) != (err == nullptr)) return fail(c, HELIOS_EINVAL, "set_observation: obs and obs_err must both be given or both NULL");
+    const double nu_first = c->nu0, nu_last = c->nu0 + c->dnu * (c->nNu - 1), tol = 1e-9 * c->dnu;
+    std::vector<double> e(edges, edges + J + 1);
+    for (int j = 0; j <= J; ++j) {
+        if (!std::isfinite(e[j]) || e[j] < nu_first - tol || e[j] > nu_last + tol)
+            return fail(c, HELIOS_EINVAL, "set_observation: bin edge %d = %g outside the grid [%g, %g]", j, e[j], nu_first, nu_last);
+        e[j] = std::fmin(std::fmax(e[j], nu_first), nu_last);
+        if (j > 0 && !(e[j] > e[j - 1])) return fail(c, HELIOS_EINVAL, "set_observation: bin edges not strictly ascending at %d", j);
+    }
+    if (obs) for (int j = 0; j < J; ++j)
+        if (!std::isfinite(obs[j]) || !(err[j] > 0) || !std::isfinite(err[j]))
+            return fail(c, HELIOS_EINVAL, "set_observation: obs/obs_err[%d] invalid", j);
+    if (inst_sigma) for (int k = 0; k < c->nNu; ++k)
+        if (!(inst_sigma[k] >= 0) || !std::isfinite(inst_sigma[k]))
+            return fail(c, HELIOS_EINVAL, "set_observation: inst_sigma[%d] invalid", k);
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_obs = c->have_data = false;
+    c->J = J;
+
+    // band extents of each row of W (marshalling: which grid points can contribute)
+    std::vector<int> row_ptr(J + 1, 0), row_lo(J), klo(J), khi(J);
+    for (int j = 0; j < J; ++j) {
+        int a = (int)std::floor((e[j] - c->nu0) / c->dnu), b = (int)std::ceil((e[j + 1] - c->nu0) / c->dnu);
+        a = a < 0 ? 0 : a; b = b > c->nNu - 1 ? c->nNu - 1 : b;
+        klo[j] = a; khi[j] = b;
+        int reach = 0;
+        if (inst_sigma) for (int k = a; k <= b; ++k) {
+            int r = (int)std::ceil(5.0 * inst_sigma[k] / c->dnu) + 1;
+            reach = r > reach ? r : reach;
+        }
+        int lo = a - reach < 0 ? 0 : a - reach, hi = b + reach > c->nNu - 1 ? c->nNu - 1 : b + reach;
+        row_lo[j] = lo;
+        row_ptr[j + 1] = row_ptr[j] + (hi - lo + 1);
+    }
+    int* d_klo = nullptr; int* d_khi = nullptr; double* d_sig = nullptr; double* d_norm = nullptr;
+    std::vector<double> sig;
+    if (inst_sigma) sig.assign(inst_sigma, inst_sigma + c->nNu);
+    CU_TRY(c, upload(c->d_edges, e, c->stream));
+    CU_TRY(c, upload(c->d_row_ptr, row_ptr, c->stream));
+    CU_TRY(c, upload(c->d_row_lo, row_lo, c->stream));
+    CU_TRY(c, upload(d_klo, klo, c->stream));
+    CU_TRY(c, upload(d_khi, khi, c->stream));
+    if (inst_sigma) CU_TRY(c, upload(d_sig, sig, c->stream));
+    CU_TRY(c, cudaMalloc(&d_norm, sizeof(double) * c->nNu));
+    dfree(c->d_W);
+    CU_TRY(c, cudaMalloc(&c->d_W, sizeof(float) * (size_t)row_ptr[J]));
+    ObsBuildArgs ba{c->nNu, J, c->nu0, c->dnu, c->d_edges, d_sig, d_norm, c->d_row_ptr, c->d_row_lo, d_klo, d_khi, c->d_W};
+    k_conv_norm<<<(c->nNu + 127) / 128, 128, 0, c->stream>>>(ba);
+    int max_len = 0;
+    for (int j = 0; j < J; ++j) max_len = std::max(max_len, row_ptr[j + 1] - row_ptr[j]);
+    k_build_W<<<dim3((max_len + 127) / 128, J), 128, 0, c->stream>>>(ba);
+    c->n_launches += 2;
+    CU_TRY(c, cudaGetLastError());
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    dfree(d_klo); dfree(d_khi); dfree(d_sig); dfree(d_norm);
+
+    if (obs) {
+        std::vector<double> o(obs, obs + J), i2v(J);
+        double cst = 0.0;
+        for (int j = 0; j < J; ++j) {
+            i2v[j] = 1.0 / (2.0 * err[j] * err[j]);
+            cst += -0.5 * std::log(2.0 * kPi * err[j] * err[j]);
+        }
+        c->logl_const = cst;
+        CU_TRY(c, upload(c->d_obs, o, c->stream));
+        CU_TRY(c, upload(c->d_inv2var, i2v, c->stream));
+        c->have_data = true;
+    }
+    c->have_obs = true;
+    c->cap_B = 0;    // staging buffers depend on J
+    return HELIOS_OK;
+}
+
+static int use_slab(const helios_ctx* c, int B) {
+    if (c->opt_kernel == 1) return 0;
+    if (c->opt_kernel == 2) return 1;
+    return slab_supported(c->S, c->C, c->nT, c->A) && B >= 16;
+}
+
+int helios_reserve(helios_ctx* c, int B) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_tables || !c->have_atmo) return fail(c, HELIOS_ESTATE, "reserve: tables and atmosphere must be set first");
+    if (B < 1 || B > 65535) return fail(c, HELIOS_EINVAL, "batch %d out of range (1..65535)", B);
+    if (B <= c->cap_B) return HELIOS_OK;
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag);
+    dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
+    c->cap_B = 0;
+    const int rf = std::max(direct_rec_floats(c->S, c->C), slab_rec_floats(c->S + c->C));
+    c->flux_stride = c->stride;
+    CU_TRY(c, cudaMalloc(&c->d_rec, sizeof(float) * (size_t)B * c->L * rf));
+    CU_TRY(c, cudaMalloc(&c->d_flux, sizeof(float) * (size_t)B * c->flux_stride));
+    CU_TRY(c, cudaMalloc(&c->d_scale, sizeof(float) * B));
+    CU_TRY(c, cudaMalloc(&c->d_flag, sizeof(int) * B));
+    CU_TRY(c, cudaMalloc(&c->d_params_stage, sizeof(double) * (size_t)B * (2 + c->K + c->S)));
+    CU_TRY(c, cudaMalloc(&c->d_spectra_stage, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
+    CU_TRY(c, cudaMalloc(&c->d_logl_stage, sizeof(double) * B));
+    c->cap_B = B;
+    return HELIOS_OK;
+}
+
+// steps 0-4: params -> flux (DEVICE [B][flux_stride])
+static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride) {
+    const int slab = use_slab(c, B);
+    const int rf = slab ? slab_rec_floats(c->S + c->C) : direct_rec_floats(c->S, c->C);
+    PrepArgs pa{};
+    pa.params = params; pa.B = B; pa.P = 2 + c->K + c->S; pa.K = c->K; pa.S = c->S; pa.C = c->C; pa.L = c->L;
+    pa.nT = c->nT; pa.nP = c->nP; pa.T_grid = c->d_Tgrid; pa.lvl_p_bar = c->d_lvl_p; pa.lvl_knot = c->d_lvl_knot;
+    pa.lvl_xi = c->d_lvl_xi; pa.lvl_ip = c->d_lvl_ip; pa.lvl_u = c->d_lvl_u; pa.lvl_pclamp = c->d_lvl_pclamp;
+    pa.lvl_lnratio = c->d_lvl_lnratio; pa.mmw = c->mmw; pa.he_to_h2 = c->he_to_h2; pa.flux_const = c->flux_const;
+    pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
+    pa.counters = c->d_counters;
+    k_prep<<<(B * c->L + 127) / 128, 128, 0, c->stream>>>(pa);
+    c->n_launches += 1;
+    CU_TRY(c, cudaGetLastError());
+
+    if (slab) {
+        SlabArgs sa{};
+        sa.sigma = c->d_sigma; sa.cia = c->d_cia; sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nP = c->nP; sa.nNu = c->nNu;
+        sa.L = c->L; sa.B = B; sa.stride = c->stride; sa.lvl_ip = c->d_lvl_ip; sa.lvl_u = c->d_lvl_uf; sa.rec = c->d_rec;
+        sa.rec_floats = rf; sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu;
+        sa.flux = flux; sa.flux_stride = flux_stride; sa.ang = c->ang;
+        int nl = 0;
+        cudaError_t e = launch_rt_slab(sa, c->A, c->opt_models_per_cta, c->num_sms, c->stream, &nl);
+        c->n_launches += nl;
+        if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "slab kernel launch failed: %s", cudaGetErrorString(e));
+        return HELIOS_OK;
+    }
+    DirectArgs da{};
+    da.sigma = c->d_sigma; da.cia = c->d_cia; da.S = c->S; da.C = c->C; da.nT = c->nT; da.nP = c->nP; da.nNu = c->nNu;
+    da.L = c->L; da.stride = c->stride; da.rec = c->d_rec; da.rec_floats = rf; da.model_scale = c->d_scale;
+    da.model_flag = c->d_flag; da.nu0 = c->nu0; da.dnu = c->dnu; da.flux = flux; da.flux_stride = flux_stride; da.ang = c->ang;
+    const size_t smem = sizeof(float) * (size_t)c->L * rf;
+    const dim3 grid((c->nNu + kDirectThreads - 1) / kDirectThreads, B);
+#define HELIOS_DIRECT_CASE(N)                                                                               \
+    case N:                                                                                                 \
+        if (smem > 48 * 1024) CU_TRY(c, cudaFuncSetAttribute(k_rt_direct<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        k_rt_direct<N><<<grid, kDirectThreads, smem, c->stream>>>(da);                                      \
+        break;
+    switch (c->A) {
+        HELIOS_DIRECT_CASE(1) HELIOS_DIRECT_CASE(2) HELIOS_DIRECT_CASE(3) HELIOS_DIRECT_CASE(4)
+        HELIOS_DIRECT_CASE(5) HELIOS_DIRECT_CASE(6) HELIOS_DIRECT_CASE(7) HELIOS_DIRECT_CASE(8)
+        default: return fail(c, HELIOS_EINVAL, "n_angles %d", c->A);
+    }
+#undef HELIOS_DIRECT_CASE
+    c->n_launches += 1;
+    CU_TRY(c, cudaGetLastError());
+    return HELIOS_OK;
+}
+
+static int check_ready(helios_ctx* c, int B, const double* params, bool need_obs, bool need_data) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_tables || !c->have_atmo) return fail(c, HELIOS_ESTATE, "tables and atmosphere must be set first");
+    if (need_obs && !c->have_obs) return fail(c, HELIOS_ESTATE, "observation grid not set (helios_set_observation)");
+    if (need_data && !c->have_data) return fail(c, HELIOS_ESTATE, "logL requested but the observation has no data");
+    if (B < 1 || B > 65535) return fail(c, HELIOS_EINVAL, "batch %d out of range (1..65535)", B);
+    if (!params) return fail(c, HELIOS_EINVAL, "params is NULL");
+    if ((size_t)c->L * std::max(direct_rec_floats(c->S, c->C), 4) * sizeof(float) > 200 * 1024)
+        return fail(c, HELIOS_EINVAL, "n_levels x record size exceeds shared memory");
+    return HELIOS_OK;
+}
+
+int helios_forward_highres(helios_ctx* c, int B, const double* params, float* flux_out) {
+    int rc = check_ready(c, B, params, false, false);
+    if (rc) return rc;
+    if (!flux_out) return fail(c, HELIOS_EINVAL, "flux_out is NULL");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if ((rc = helios_reserve(c, B))) return rc;
+    c->n_models += B;
+    return run_flux(c, B, params, flux_out, c->nNu);
+}
+
+int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spectra_out, double* logl_out) {
+    int rc = check_ready(c, B, params, true, logl_out != nullptr);
+    if (rc) return rc;
+    if (!spectra_out && !logl_out) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if ((rc = helios_reserve(c, B))) return rc;
+    c->n_models += B;
+    if ((rc = run_flux(c, B, params, c->d_flux, c->flux_stride))) return rc;
+    ObsApplyArgs oa{};
+    oa.J = c->J; oa.row_ptr = c->d_row_ptr; oa.row_lo = c->d_row_lo; oa.W = c->d_W; oa.flux = c->d_flux;
+    oa.flux_stride = c->flux_stride; oa.model_flag = c->d_flag; oa.obs = c->d_obs; oa.inv2var = c->d_inv2var;
+    oa.logl_const = c->logl_const; oa.spectra = spectra_out; oa.logl = logl_out;
+    k_obs_apply<<<B, kObsThreads, 0, c->stream>>>(oa);
+    c->n_launches += 1;
+    CU_TRY(c, cudaGetLastError());
+    return HELIOS_OK;
+}
+
+int helios_loglike_batch(helios_ctx* c, int B, const double* params, double* logl_out) {
+    if (c && !logl_out) return fail(c, HELIOS_EINVAL, "logl_out is NULL");
+    return helios_forward_batch(c, B, params, nullptr, logl_out);
+}
+
+int helios_forward_batch_host(helios_ctx* c, int B, const double* params_host, float* spectra_host, double* logl_host) {
+    int rc = check_ready(c, B, params_host, true, logl_host != nullptr);
+    if (rc) return rc;
+    if (!spectra_host && !logl_host) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if ((rc = helios_reserve(c, B))) return rc;
+    const size_t P = 2 + c->K + c->S;
+    CU_TRY(c, cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * P, cudaMemcpyHostToDevice, c->stream));
+    rc = helios_forward_batch(c, B, c->d_params_stage, spectra_host ? c->d_spectra_stage : nullptr,
+                              logl_host ? c->d_logl_stage : nullptr);
+    if (rc) return rc;
+    if (spectra_host)
+        CU_TRY(c, cudaMemcpyAsync(spectra_host, c->d_spectra_stage, sizeof(float) * (size_t)B * c->J, cudaMemcpyDeviceToHost, c->stream));
+    if (logl_host)
+        CU_TRY(c, cudaMemcpyAsync(logl_host, c->d_logl_stage, sizeof(double) * B, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return HELIOS_OK;
+}
+
+int helios_get_stats(helios_ctx* c, helios_stats* out, int reset) {
+    if (!c || !out) return HELIOS_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    unsigned long long h[2] = {0, 0};
+    CU_TRY(c, cudaMemcpyAsync(h, c->d_counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    out->n_clamped = h[0]; out->n_nonfinite = h[1]; out->n_models = c->n_models; out->n_launches = c->n_launches;
+    if (reset) {
+        CU_TRY(c, cudaMemsetAsync(c->d_counters, 0, sizeof h, c->stream));
+        c->n_models = 0; c->n_launches = 0;
+    }
+    return HELIOS_OK;
+}
+
+}  // extern "C"

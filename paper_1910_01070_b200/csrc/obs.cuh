@@ -1,0 +1,136 @@
+// obs.cuh -- step 5 of the hot path: instrument profile (Eq. 17,
+// PAPER.md:229-235), binning and likelihood (Eq. 19,
+// PAPER.md:267-270), fused.
+//
+// "Convolve on the native grid, then bin-average" is linear and model-independent,
+// so helios_set_observation() builds ONE banded operator W[J][band] on the device
+// (fp64 arithmetic, fp32 storage) and the per-batch kernel applies it:
+//     M_j = sum_i W_ji F_i,   W_ji = sum_k b_jk c_ki
+//   c_ki = g(nu_i - nu_k; sigma_k) / sum_i' g(nu_i' - nu_k; sigma_k), |nu_i - nu_k| <= 5 sigma_k
+//   b_jk = (1/(e_{j+1} - e_j)) * integral over the bin of the hat function of grid point k
+//          (= the weight of F_d[k] in the bin mean of the piecewise-linear interpolant).
+// DESIGN.md R15, R17, R18.
+#pragma once
+#include "common.cuh"
+
+namespace helios {
+
+struct ObsBuildArgs {
+    int nNu, J;
+    double nu0, dnu;
+    const double* edges;       // DEVICE [J+1]
+    const double* inst_sigma;  // DEVICE [nNu] or nullptr
+    double* conv_norm;         // DEVICE [nNu]  sum of Gaussian weights actually used
+    const int* row_ptr;        // DEVICE [J+1]
+    const int* row_lo;         // DEVICE [J]    first grid index of the row's band
+    const int* row_klo;        // DEVICE [J]    first / last grid point with non-zero bin weight
+    const int* row_khi;
+    float* W;                  // DEVICE [row_ptr[J]]
+};
+
+__global__ void k_conv_norm(ObsBuildArgs a) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= a.nNu) return;
+    double sg = a.inst_sigma ? a.inst_sigma[k] : 0.0;
+    if (!(sg > 0.0)) { a.conv_norm[k] = 1.0; return; }
+    int reach = (int)ceil(5.0 * sg / a.dnu) + 1;
+    int lo = max(0, k - reach), hi = min(a.nNu - 1, k + reach);
+    double nu_k = a.nu0 + a.dnu * k;
+    double sum = 0.0;
+    for (int i = lo; i <= hi; ++i) {
+        double d = (a.nu0 + a.dnu * i) - nu_k;
+        if (fabs(d) <= 5.0 * sg) sum += exp(-d * d / (2.0 * sg * sg));
+    }
+    a.conv_norm[k] = sum;
+}
+
+// integral of the unit hat function centred at 0 with half-width 1, from -inf to s
+__device__ __forceinline__ double hat_cdf(double s) {
+    if (s <= -1.0) return 0.0;
+    if (s >= 1.0) return 1.0;
+    return s < 0.0 ? 0.5 * (1.0 + s) * (1.0 + s) : 1.0 - 0.5 * (1.0 - s) * (1.0 - s);
+}
+
+__global__ void k_build_W(ObsBuildArgs a) {
+    const int j = blockIdx.y;
+    const int len = a.row_ptr[j + 1] - a.row_ptr[j];
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= len) return;
+    const int i = a.row_lo[j] + e;
+    const double ea = a.edges[j], eb = a.edges[j + 1];
+    const double nu_i = a.nu0 + a.dnu * i;
+    double w = 0.0;
+    for (int k = a.row_klo[j]; k <= a.row_khi[j]; ++k) {
+        const double nu_k = a.nu0 + a.dnu * k;
+        const double bjk = (hat_cdf((eb - nu_k) / a.dnu) - hat_cdf((ea - nu_k) / a.dnu)) * a.dnu / (eb - ea);
+        if (bjk == 0.0) continue;
+        const double sg = a.inst_sigma ? a.inst_sigma[k] : 0.0;
+        if (!(sg > 0.0)) { if (i == k) w += bjk; continue; }
+        const double d = nu_i - nu_k;
+        if (fabs(d) <= 5.0 * sg) w += bjk * exp(-d * d / (2.0 * sg * sg)) / a.conv_norm[k];
+    }
+    a.W[a.row_ptr[j] + e] = (float)w;
+}
+
+struct ObsApplyArgs {
+    int J;
+    const int* row_ptr;
+    const int* row_lo;
+    const float* W;
+    const float* flux;        // DEVICE [B][flux_stride]
+    long long flux_stride;
+    const int* model_flag;
+    const double* obs;        // DEVICE [J] or nullptr
+    const double* inv2var;    // DEVICE [J]  1 / (2 sigma_j^2)
+    double logl_const;        // -1/2 sum_j ln(2 pi sigma_j^2)
+    float* spectra;           // DEVICE [B][J] or nullptr
+    double* logl;             // DEVICE [B] or nullptr
+};
+
+constexpr int kObsThreads = 256;
+
+// One CTA per model.  Each warp owns bins j = warp, warp + 8, ...: lanes stride the band,
+// a shuffle tree finishes M_j, lane 0 adds the chi-square term in fp64.  The per-warp
+// partial sums are combined in a fixed order, so logL is bitwise reproducible.
+__global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
+    __shared__ double warp_sum[kObsThreads / 32];
+    const int b = blockIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool bad = a.model_flag[b] != 0;
+    const float* F = a.flux + (size_t)b * a.flux_stride;
+    double chi2 = 0.0;
+    for (int j = warp; j < a.J; j += kObsThreads / 32) {
+        const int p0 = a.row_ptr[j], len = a.row_ptr[j + 1] - p0;
+        const float* w = a.W + p0;
+        const float* f = F + a.row_lo[j];
+        float acc0 = 0.0f, acc1 = 0.0f;
+        int i = lane;
+        for (; i + 32 < len; i += 64) {
+            acc0 = fmaf(w[i], f[i], acc0);
+            acc1 = fmaf(w[i + 32], f[i + 32], acc1);
+        }
+        if (i < len) acc0 = fmaf(w[i], f[i], acc0);
+        float acc = acc0 + acc1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) {
+            if (bad) acc = __int_as_float(0x7fc00000);
+            if (a.spectra) a.spectra[(size_t)b * a.J + j] = acc;
+            if (a.logl) {
+                double r = a.obs[j] - (double)acc;
+                chi2 += r * r * a.inv2var[j];
+            }
+        }
+    }
+    if (a.logl) {
+        if (lane == 0) warp_sum[warp] = chi2;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s = 0.0;
+            for (int w = 0; w < kObsThreads / 32; ++w) s += warp_sum[w];
+            a.logl[b] = bad ? -CUDART_INF : a.logl_const - s;
+        }
+    }
+}
+
+}  // namespace helios

@@ -1,0 +1,120 @@
+// prep.cuh -- step 0 of the hot path: per (model, level) profile
+// quantities, interpolation cells/weights and number-density-weighted tap weights.
+// fp64 arithmetic, fp32 results.  PAPER.md:55 (levels), 174-221 (first-order
+// elements), 484 (isoprofiles, H2/He fill), 241 (interpolation).
+#pragma once
+#include "common.cuh"
+
+namespace helios {
+
+struct PrepArgs {
+    const double* params;     // DEVICE [B][P]
+    int B, P, K, S, C, L, nT, nP;
+    const double* T_grid;     // DEVICE [nT]
+    const double* lvl_p_bar;  // DEVICE [L]
+    const int*    lvl_knot;   // DEVICE [L]  element index of the level
+    const double* lvl_xi;     // DEVICE [L]  reference-element coordinate in [0,1]
+    const int*    lvl_ip;     // DEVICE [L]  pressure cell
+    const double* lvl_u;      // DEVICE [L]  pressure weight in [0,1]
+    const int*    lvl_pclamp; // DEVICE [L]  1 if the level pressure is outside the table
+    const double* lvl_lnratio;// DEVICE [L]  ln(p_l / p_{l+1}) (0 for the top level)
+    double mmw, he_to_h2, flux_const;
+    float* rec;               // DEVICE [B][L][rec_floats]
+    int rec_floats;
+    int slab_layout;          // 0: direct (4 taps / species), 1: slab (2 taps / row)
+    float* model_scale;       // DEVICE [B]  f * flux_const * 2 pi
+    int*   model_flag;        // DEVICE [B]  1 = non-finite parameter
+    unsigned long long* counters;  // [0] clamped pairs, [1] non-finite models
+};
+
+__device__ __forceinline__ double knot_temperature(const double* th_knots, int K, int k, double xi) {
+    if (K == 1) return th_knots[0];
+    return th_knots[k] * (1.0 - xi) + th_knots[k + 1] * xi;
+}
+
+__global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= a.B * a.L) return;
+    int b = idx / a.L, l = idx - b * a.L;
+    const double* th = a.params + (size_t)b * a.P;
+
+    bool finite = true;
+    for (int i = 0; i < a.P; ++i) finite = finite && isfinite(th[i]);
+    float* rec = a.rec + ((size_t)b * a.L + l) * a.rec_floats;
+    if (l == 0) {
+        a.model_flag[b] = finite ? 0 : 1;
+        a.model_scale[b] = finite ? (float)(th[1] * a.flux_const * 2.0 * kPi) : 0.0f;
+        if (!finite) atomicAdd(&a.counters[1], 1ULL);
+    }
+    if (!finite) {
+        for (int i = 0; i < a.rec_floats; ++i) rec[i] = 0.0f;
+        return;
+    }
+
+    const double g = pow(10.0, th[0]);
+    const double* knots = th + 2;
+    const double* lvmr = th + 2 + a.K;
+
+    const double T = knot_temperature(knots, a.K, a.lvl_knot[l], a.lvl_xi[l]);
+    const double p = a.lvl_p_bar[l];
+
+    // temperature cell: largest iT with T_grid[iT] <= T, clamped to [0, nT-2]
+    int iT = 0;
+    for (int k = 0; k < a.nT; ++k) if (a.T_grid[k] <= T) iT = k;
+    if (iT > a.nT - 2) iT = a.nT - 2;
+    double t = (T - a.T_grid[iT]) / (a.T_grid[iT + 1] - a.T_grid[iT]);
+    int clamped = a.lvl_pclamp[l];
+    if (t < 0.0) { t = 0.0; clamped = 1; }
+    if (t > 1.0) { t = 1.0; clamped = 1; }
+    if (clamped) atomicAdd(&a.counters[0], 1ULL);
+    const double u = a.lvl_u[l];
+
+    const double n = p * kBarCgs / (kBoltzmann * T);     // cm^-3
+    double xsum = 0.0;
+    for (int s = 0; s < a.S; ++s) xsum += pow(10.0, lvmr[s]);
+    const double x_bg = 1.0 - xsum;
+    const double x_h2 = x_bg / (1.0 + a.he_to_h2);
+    const double x_he = x_bg * a.he_to_h2 / (1.0 + a.he_to_h2);
+    const double am = n / kAmagat;
+
+    int o = 0;
+    if (!a.slab_layout) {
+        for (int s = 0; s < a.S; ++s) {
+            double w = n * pow(10.0, lvmr[s]);
+            rec[o++] = (float)(w * (1.0 - t) * (1.0 - u));
+            rec[o++] = (float)(w * (1.0 - t) * u);
+            rec[o++] = (float)(w * t * (1.0 - u));
+            rec[o++] = (float)(w * t * u);
+        }
+    } else {
+        for (int s = 0; s < a.S; ++s) {
+            double w = n * pow(10.0, lvmr[s]);
+            rec[o++] = (float)(w * (1.0 - t));
+            rec[o++] = (float)(w * t);
+        }
+    }
+    for (int c = 0; c < a.C; ++c) {
+        double w = am * am * x_h2 * (c == 0 ? x_h2 : x_he);
+        rec[o++] = (float)(w * (1.0 - t));
+        rec[o++] = (float)(w * t);
+    }
+    // Planck exponent scale and half layer thickness (hydrostatic, ideal gas; R5)
+    rec[o++] = (float)(kC2 * kLog2e / T);
+    double hdz = 0.0;
+    if (l + 1 < a.L) {
+        double T_up = knot_temperature(knots, a.K, a.lvl_knot[l + 1], a.lvl_xi[l + 1]);
+        double dz = kBoltzmann * 0.5 * (T + T_up) / (a.mmw * kAtomicMass * g) * a.lvl_lnratio[l];
+        hdz = 0.5 * dz;
+    }
+    rec[o++] = (float)hdz;
+    if (!a.slab_layout) {
+        rec[o++] = __int_as_float(iT * a.nP + a.lvl_ip[l]);
+        rec[o++] = __int_as_float(iT);
+    } else {
+        rec[o++] = __int_as_float(iT);
+        rec[o++] = 0.0f;
+    }
+    while (o < a.rec_floats) rec[o++] = 0.0f;
+}
+
+}  // namespace helios
