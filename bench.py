@@ -1,0 +1,319 @@
+"""bench.py -- throughput of the batched Helios-r2 forward model on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl reference]
+
+A "step" is one pass of the whole hot path (profile prep -> interpolate ->
+optical depth -> RT -> convolve/bin/chi-square) over one batch of synthetic
+input, through the C ABI (helios_forward_batch; spectra and logL written).
+Default workload: BASELINE.json configs[2] (JWST-like broadband, B = 256),
+the configuration the "batch >= 256" target of north_star is quoted on.
+Prints ONE JSON line.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads  # noqa: E402
+
+# B200: 148 SMs x 128 FP32 lanes x 1.965 GHz (guide unit counts, clocks.max.sm), 1 FMA = 2 flop
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+HBM_NOMINAL_GBS = 8000.0
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
+# ncu --set full capture summarised in profiles/ (None until captured for this workload).
+NCU_TRAFFIC_BYTES = {}
+
+
+def algorithmic_ops(cfg):
+    """FMA-class fp32 ops and MUFU ops per (model, nu) point, as the METHOD defines them
+    (4-tap bilinear per species, 2-tap per CIA pair)."""
+    L, S, C, A = cfg.n_levels, cfg.n_species, cfg.n_cia, cfg.n_angles
+    fma = L * (4 * S + 2 * C) + 2 * (L - 1) + 4 * L + 6 * (L - 1) * A
+    mufu = 2 * L + (L - 1) * (A + 1)
+    return fma, mufu
+
+
+def must_move_bytes(cfg, B):
+    """BASELINE.json's HBM roofline numerator: table bytes + parameter and output bytes."""
+    table = 4 * cfg.n_nu * len(cfg.T_grid) * (cfg.n_species * len(cfg.log10p_grid) + cfg.n_cia)
+    P = 2 + cfg.n_knots + cfg.n_species
+    return table + B * P * 8 + B * cfg.n_bins * 4 + B * 8
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return json.load(open(path)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.tmp = None
+
+    def start(self):
+        try:
+            self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.tmp.flush()
+        rows = [r.strip().split(",") for r in open(self.tmp.name) if r.strip()]
+        os.unlink(self.tmp.name)
+        sm, reasons = [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                out["sm_max_mhz"] = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.strip().lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+        out["reasons"] = sorted(reasons)
+        out["samples"] = len(sm)
+        return out
+
+
+def oracle_sample_size(cfg, cores):
+    """Bounded sample: about 10-30 s of CPU work (measured ~0.8 core-s per model at configs[2])."""
+    per_model = 6e-9 * cfg.n_nu * cfg.n_levels * (4 * cfg.n_species + 2 * cfg.n_cia + 3 * cfg.n_angles + 6)
+    n = int(max(1, min(cfg.batch, round(20.0 / max(per_model, 1e-3)))))
+    return max(min(n, cfg.batch), min(cores, cfg.batch))
+
+
+def time_oracle(wl, n_models, repeats=1):
+    """The oracle as it stands (never tuned), all host cores, table generation excluded."""
+    import oracle
+    params = np.ascontiguousarray(wl.params[:n_models])
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        oracle.forward_workload(wl, params=params, want_spectra=True, want_logl=wl.obs is not None)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return best, oracle.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the fp64 CPU oracle on this box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = workloads.get_config(args.config)
+    wl = workloads.make_workload(args.config, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls)
+    import oracle
+    cores = oracle.max_threads()
+    n = oracle_sample_size(cfg, cores)
+    n = max(1, min(n, max(cores, n // max(1, args.steps // 2))))   # keep K+W steps within minutes
+    for _ in range(args.warmup):
+        time_oracle(wl, min(n, cores))
+    t = [time_oracle(wl, n)[0] for _ in range(args.steps)]
+    dt = float(np.mean(t))
+    value = n / dt
+    sample = f"{n} of {cfg.batch} models of configs[{cfg.index}] per step, all nu/levels/bins"
+    line = {
+        "impl": "reference", "metric": "forward_models_per_s", "value": value, "unit": "models/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "batch_per_step": n, "n_nu": cfg.n_nu,
+                   "n_levels": cfg.n_levels, "n_species": cfg.n_species, "n_cia": cfg.n_cia,
+                   "n_angles": cfg.n_angles, "n_bins": cfg.n_bins},
+        "points_per_s": value * cfg.n_nu,
+        "cpu_baseline": {"value": value, "unit": "models/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "models/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1910_01070_b200 import Helios
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    cfg = workloads.get_config(args.config)
+    n_calls = cfg.n_calls                       # configs[4]: 16 back-to-back calls per step
+    B_call = cfg.batch // n_calls
+    wl = workloads.make_workload(args.config, batch=cfg.batch, device="cuda")
+    # weak scaling over the batch: every rank evaluates its own cfg.batch models against replicated
+    # tables; rank r draws different parameter vectors.
+    if rank > 0:
+        rng = np.random.default_rng([cfg.seed, rank])
+        wl.params = wl.params[rng.permutation(cfg.batch)]
+    want_spec = cfg.spectra_out
+
+    h = Helios(local)
+    h.setup_workload(wl)
+    h.set_kernel(args.kernel, args.models_per_cta)
+    P = wl.params.shape[1]
+    p_dev = torch.as_tensor(wl.params, device=dev)
+    spec = torch.empty((cfg.batch, cfg.n_bins), dtype=torch.float32, device=dev) if want_spec else None
+    logl = torch.empty((cfg.batch,), dtype=torch.float64, device=dev)
+    p_host = torch.as_tensor(wl.params).pin_memory()
+    spec_host = torch.empty((cfg.batch, cfg.n_bins), dtype=torch.float32).pin_memory() if want_spec else None
+    logl_host = torch.empty((cfg.batch,), dtype=torch.float64).pin_memory()
+
+    from paper_1910_01070_b200 import helios_forward_batch, helios_forward_batch_host
+
+    def step_device():
+        for c in range(n_calls):
+            s = slice(c * B_call, (c + 1) * B_call)
+            helios_forward_batch(h.ctx, p_dev[s], spec[s] if want_spec else None, logl[s])
+
+    def step_host():
+        for c in range(n_calls):
+            s = slice(c * B_call, (c + 1) * B_call)
+            helios_forward_batch_host(h.ctx, p_host[s], spec_host[s] if want_spec else None, logl_host[s])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, sampler=None):
+        barrier()
+        if sampler:
+            sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        barrier()
+        clocks = sampler.stop() if sampler else None
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms, clocks
+
+    for _ in range(max(args.warmup, 3)):
+        step_device()
+    h.stats(reset=True)
+    h.set_timing(True)
+    ms, clocks = timed(step_device, args.steps, ClockSampler(local) if rank == 0 else None)
+    stage = h.stage_ms()
+    st = h.stats(reset=True)
+    h.set_timing(False)
+    for _ in range(2):
+        step_host()
+    ms_host, _ = timed(step_host, args.steps)
+
+    ms_step = ms / args.steps
+    total_models = cfg.batch * world
+    value = total_models / (ms_step * 1e-3)
+    e2e_value = total_models / (ms_host / args.steps * 1e-3)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks, peak_src = measured_peaks()
+    fma, mufu = algorithmic_ops(cfg)
+    rt_ms = stage["rt_ms"]                                    # per call, CUDA events on the ctx stream
+    ach_tflops = 2.0 * fma * B_call * cfg.n_nu / (rt_ms * 1e-3) / 1e12
+    bytes_move = must_move_bytes(cfg, B_call)
+    line = {
+        "metric": "forward_models_per_s", "value": value, "unit": "models/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "batch": cfg.batch, "calls_per_step": n_calls,
+                   "n_nu": cfg.n_nu, "n_levels": cfg.n_levels, "n_species": cfg.n_species, "n_cia": cfg.n_cia,
+                   "n_angles": cfg.n_angles, "n_bins": cfg.n_bins, "spectra_written": bool(want_spec),
+                   "parallelism": f"batch-sharded x{world}, tables replicated",
+                   "l2": "opacity table (%.0f MB) exceeds the 126 MB L2; no flush" % (bytes_move / 1e6),
+                   "kernel": {0: "auto", 1: "direct", 2: "slab"}[args.kernel]},
+        "points_per_s": value * cfg.n_nu,
+        "stage_ms_per_call": stage,
+        "roofline": {"bound": "alu", "kernel": "fused interpolate+tau+RT", "achieved": ach_tflops,
+                     "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tflops / ALU_PEAK_TFLOPS,
+                     "traffic": NCU_TRAFFIC_BYTES.get(cfg.index),
+                     "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md)",
+                     "algorithmic_fma_per_point": fma, "algorithmic_mufu_per_point": mufu},
+        "hbm_roofline": {"must_move_bytes_per_call": bytes_move,
+                         "achieved_gbs": bytes_move / (ms_step / n_calls * 1e-3) / 1e9,
+                         "frac_of_8TBs": bytes_move / (ms_step / n_calls * 1e-3) / 1e9 / HBM_NOMINAL_GBS,
+                         "frac_of_measured": bytes_move / (ms_step / n_calls * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                         "measured_peak_gbs": peaks["hbm_gbs"], "peak_source": peak_src},
+        "e2e": {"value": e2e_value, "unit": "models/s", "h2d_bytes_per_step": cfg.batch * P * 8,
+                "d2h_bytes_per_step": cfg.batch * ((cfg.n_bins * 4 if want_spec else 0) + 8)},
+        "gpu_launches": st["n_launches"],
+        "clocks": clocks,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        n = oracle_sample_size(cfg, oracle.max_threads())
+        dt, cores = time_oracle(wl, n)
+        line["cpu_baseline"] = {"value": n / dt, "unit": "models/s", "cores": cores, "kind": "oracle",
+                                "sample": f"first {n} of {cfg.batch} models of configs[{cfg.index}], "
+                                          f"all nu/levels/bins, {dt:.1f} s wall"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 slab")
+    ap.add_argument("--models-per-cta", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -44,6 +44,7 @@ enum {
 /* helios_set_option keys */
 #define HELIOS_OPT_KERNEL      1   /* 0 = auto, 1 = direct (4-tap, global loads), 2 = slab (staged, large batch) */
 #define HELIOS_OPT_MODELS_PER_CTA 2/* slab kernel: models per CTA (0 = auto) */
+#define HELIOS_OPT_TIMING      3   /* 1 = bracket every stage of the next calls with CUDA events on the context's stream */
 
 typedef struct helios_stats {
     unsigned long long n_clamped;      /* (model, level) pairs whose (T, p) fell outside the table and were clamped */
@@ -129,6 +130,11 @@ int helios_forward_batch_host(helios_ctx* ctx, int B, const double* params_host,
 
 /* Copies the counters (synchronises the stream); reset != 0 clears them. */
 int helios_get_stats(helios_ctx* ctx, helios_stats* out, int reset);
+/* Average device time per call of each stage (prep, fused interpolate+RT kernel, fused
+ * convolve/bin/chi-square kernel) over the calls made since HELIOS_OPT_TIMING was set to 1
+ * (at most the last 64), from CUDA events recorded on the context's stream.
+ * HOST out: stage_ms[3], n_calls.  Synchronises the stream. */
+int helios_get_stage_ms(helios_ctx* ctx, double* stage_ms, int* n_calls);
 /* HOST out: the angle set in use, mu[n_angles], w[n_angles]. */
 int helios_get_angles(const helios_ctx* ctx, double* mu_out, double* w_out);
 

@@ -20,6 +20,7 @@ HELIOS_EINVAL, HELIOS_ENOMEM, HELIOS_ECUDA, HELIOS_ESTATE = -1, -2, -3, -4
 HELIOS_PTRS_ON_DEVICE = 1
 HELIOS_OPT_KERNEL = 1
 HELIOS_OPT_MODELS_PER_CTA = 2
+HELIOS_OPT_TIMING = 3
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB = 0, 1, 2
 
 _dp = C.POINTER(C.c_double)
@@ -69,10 +70,12 @@ def lib() -> C.CDLL:
         L.helios_forward_batch_host.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
         L.helios_get_stats.argtypes = [_vp, C.POINTER(helios_stats), C.c_int]
         L.helios_get_angles.argtypes = [_vp, _dp, _dp]
+        L.helios_get_stage_ms.argtypes = [_vp, _dp, C.POINTER(C.c_int)]
         for name in ("helios_create", "helios_set_stream", "helios_set_option", "helios_load_opacity",
                      "helios_set_atmosphere", "helios_set_observation", "helios_reserve",
                      "helios_forward_batch", "helios_loglike_batch", "helios_forward_highres",
-                     "helios_forward_batch_host", "helios_get_stats", "helios_get_angles"):
+                     "helios_forward_batch_host", "helios_get_stats", "helios_get_angles",
+                     "helios_get_stage_ms"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -215,6 +218,13 @@ def helios_get_stats(ctx: int, reset: bool = False) -> dict:
     return {k: int(getattr(st, k)) for k, _ in helios_stats._fields_}
 
 
+def helios_get_stage_ms(ctx: int) -> dict:
+    ms = (C.c_double * 3)()
+    n = C.c_int()
+    _check(ctx, lib().helios_get_stage_ms(_vp(ctx), ms, C.byref(n)))
+    return {"prep_ms": ms[0], "rt_ms": ms[1], "obs_ms": ms[2], "n_calls": n.value}
+
+
 def helios_get_angles(ctx: int, n_angles: int):
     mu = np.empty(n_angles, np.float64)
     w = np.empty(n_angles, np.float64)
@@ -303,6 +313,12 @@ class Helios:
 
     def forward_batch_host(self, params_host, spectra_out_host=None, logl_out_host=None):
         helios_forward_batch_host(self.ctx, params_host, spectra_out_host, logl_out_host)
+
+    def set_timing(self, on: bool):
+        helios_set_option(self.ctx, HELIOS_OPT_TIMING, 1 if on else 0)
+
+    def stage_ms(self) -> dict:
+        return helios_get_stage_ms(self.ctx)
 
     def stats(self, reset=False):
         return helios_get_stats(self.ctx, reset)

@@ -26,15 +26,16 @@ constexpr int kMaxCia = 2;
 //   [0, 4S)        species tap weights  n x_s {(1-t)(1-u), (1-t)u, t(1-u), t u}
 //                  for table rows (iT,ip), (iT,ip+1), (iT+1,ip), (iT+1,ip+1)
 //   [4S, 4S+2C)    CIA tap weights      am^2 x_H2 x_c {(1-t), t}   rows iT, iT+1
-//   +0  planck_a   c2 log2(e) / T_l     (B_nu = c1 nu^3 E/(1-E), E = 2^(-planck_a nu))
-//   +1  hdz        dz_l / 2 of the layer between level l and l+1 (0 at the top level)
-//   +2  cell       iT*nP + ip           (int bits)
-//   +3  iT                               (int bits)
-__host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S + 2 * C + 4 + 3) & ~3; }
+//   +0  planck_a   c2 log2(e) / T_l, high part (B_nu = c1 nu^3 E/(1-E), E = 2^(-planck_a nu))
+//   +1  planck_a   low part (fp64 value minus the fp32 high part)
+//   +2  hdz        dz_l / 2 of the layer between level l and l+1 (0 at the top level)
+//   +3  cell       iT*nP + ip           (int bits)
+//   +4  iT                               (int bits)
+__host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S + 2 * C + 5 + 3) & ~3; }
 
 // Slab kernel record, fp32 (p-blend is shared by all models, so 2 taps per row):
 //   [0, 2R)  pairs {a_r, b_r}: weights of the p-blended rows iT and iT+1, r < R = S + C
-//   +0 planck_a  +1 hdz  +2 iT (int bits)  +3 unused
+//   +0 planck_a (high)  +1 planck_a (low)  +2 hdz  +3 iT (int bits)
 __host__ __device__ inline int slab_rec_floats(int R) { return (2 * R + 4 + 3) & ~3; }
 
 struct AngleSet {
@@ -57,27 +58,50 @@ __device__ __forceinline__ float rcp_approx(float x) {
     return y;
 }
 
+// E = exp(-c2 nu / T) = 2^(-a nu) with a = a_hi + a_lo and nu = nu_hi + nu_lo carried as
+// two-float numbers: the exponent reaches ~50 in the Wien tail, where one fp32 rounding of
+// a*nu alone costs 3e-6 relative in E -- enough to move logL by more than 1e-3.  The product
+// is formed exactly (FMA residual) and the sub-ulp part applied as a first-order factor.
+__device__ __forceinline__ float planck_E(float a_hi, float a_lo, float nu_hi, float nu_lo) {
+    const float p = a_hi * nu_hi;
+    float r = fmaf(a_hi, nu_hi, -p);        // exact low part of the product
+    r = fmaf(a_lo, nu_hi, r);
+    r = fmaf(a_hi, nu_lo, r);
+    const float E0 = ex2_approx(-p);
+    return fmaf(E0 * -0.69314718056f, r, E0);
+}
+
+// B_nu(T) = c1 nu^3 E / (1 - E)  (Eq. 2, per-wavenumber form; never exp(+x)).
+__device__ __forceinline__ float planck_from_E(float c1nu3, float E) {
+    return c1nu3 * (E * rcp_approx(1.0f - E));
+}
+
 // Short-characteristics update for one angle in deviation form.
 // With J = I - S(level) and dS = S_{l-1} - S_l, Eq. 4-6 read
 //   J_l = e^{-D} J_{l-1} + phi(D) dS,   phi(D) = (1 - e^{-D})/D,   D = dtau / mu  (Eq. 7)
 // (beta = 1 - phi, gamma = phi - e^{-D}).  phi is evaluated by its Taylor series for
 // D < kPhiSwitch, where (1 - e^{-D})/D cancels in fp32 (R10).
-constexpr float kPhiSwitch = 0.0625f;
+constexpr float kPhiSwitch = 0.25f;
 __device__ __forceinline__ float phi_series(float D) {
-    // 1 - D/2 + D^2/6 - D^3/24 + D^4/120 - D^5/720
-    float p = fmaf(D, -1.0f / 720.0f, 1.0f / 120.0f);
+    // 1 - D/2 + D^2/6 - D^3/24 + D^4/120 - D^5/720 + D^6/5040   (|error| < 7e-9 for D < 1/4)
+    float p = fmaf(D, 1.0f / 5040.0f, -1.0f / 720.0f);
+    p = fmaf(D, p, 1.0f / 120.0f);
     p = fmaf(D, p, -1.0f / 24.0f);
     p = fmaf(D, p, 1.0f / 6.0f);
     p = fmaf(D, p, -0.5f);
     return fmaf(D, p, 1.0f);
 }
+// Small D: e^{-D} = 1 - D phi(D) exactly, so J_l = J + phi (dS - D J): two correctly rounded
+// FMAs and no exponential.  (MUFU.EX2 results just below 1 carry a one-sided error of a
+// fraction of an ulp; through ~50 transparent layers that biased the flux by -4e-7, which
+// the absolute logL tolerance does not allow.)  Large D: hardware 2^x.
 __device__ __forceinline__ void sc_update(float& J, float dtau, float inv_dtau, float dS,
                                           float c_exp, float inv_mu, float mu) {
-    float D = dtau * inv_mu;
-    float e = ex2_approx(-dtau * c_exp);
-    float phi_big = (1.0f - e) * (mu * inv_dtau);
-    float phi = (D < kPhiSwitch) ? phi_series(D) : phi_big;
-    J = fmaf(e, J, phi * dS);
+    const float D = dtau * inv_mu;
+    const float e = ex2_approx(-dtau * c_exp);
+    const float J_big = fmaf(e, J, (1.0f - e) * (mu * inv_dtau) * dS);
+    const float J_small = fmaf(phi_series(D), fmaf(-D, J, dS), J);
+    J = (D < kPhiSwitch) ? J_small : J_big;
 }
 
 }  // namespace helios

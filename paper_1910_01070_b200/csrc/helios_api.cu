@@ -2,6 +2,7 @@
 // upload, atmosphere / observation setup, kernel launches.  sm_100a only.
 #include <math_constants.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -63,7 +64,12 @@ struct helios_ctx {
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
     // ---- options / statistics
-    int opt_kernel = 0, opt_models_per_cta = 0;
+    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0;
+    static constexpr int kTimingRing = 64;
+    cudaEvent_t ev[kTimingRing][4] = {};
+    bool ev_has_obs[kTimingRing] = {};
+    bool ev_created = false;
+    long long timed_calls = 0;
     unsigned long long n_models = 0, n_launches = 0;
 };
 
@@ -143,6 +149,7 @@ void helios_destroy(helios_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
+    if (c->ev_created) for (auto& q : c->ev) for (auto& e : q) cudaEventDestroy(e);
     free_all(c);
     delete c;
 }
@@ -164,6 +171,13 @@ int helios_set_option(helios_ctx* c, int key, int value) {
         case HELIOS_OPT_MODELS_PER_CTA:
             if (value < 0) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be >= 0");
             c->opt_models_per_cta = value; return HELIOS_OK;
+        case HELIOS_OPT_TIMING:
+            c->opt_timing = value ? 1 : 0; c->timed_calls = 0;
+            if (value && !c->ev_created) {
+                for (auto& q : c->ev) for (auto& e : q) CU_TRY(c, cudaEventCreate(&e));
+                c->ev_created = true;
+            }
+            return HELIOS_OK;
         default: return fail(c, HELIOS_EINVAL, "unknown option %d", key);
     }
 }
@@ -421,6 +435,10 @@ int helios_reserve(helios_ctx* c, int B) {
     return HELIOS_OK;
 }
 
+static inline void stamp(helios_ctx* c, int which) {
+    if (c->opt_timing) cudaEventRecord(c->ev[c->timed_calls % helios_ctx::kTimingRing][which], c->stream);
+}
+
 // steps 0-4: params -> flux (DEVICE [B][flux_stride])
 static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride) {
     const int slab = use_slab(c, B);
@@ -432,9 +450,11 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     pa.lvl_lnratio = c->d_lvl_lnratio; pa.mmw = c->mmw; pa.he_to_h2 = c->he_to_h2; pa.flux_const = c->flux_const;
     pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
     pa.counters = c->d_counters;
+    stamp(c, 0);
     k_prep<<<(B * c->L + 127) / 128, 128, 0, c->stream>>>(pa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
+    stamp(c, 1);
 
     if (slab) {
         SlabArgs sa{};
@@ -446,6 +466,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         cudaError_t e = launch_rt_slab(sa, c->A, c->opt_models_per_cta, c->num_sms, c->stream, &nl);
         c->n_launches += nl;
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "slab kernel launch failed: %s", cudaGetErrorString(e));
+        stamp(c, 2);
         return HELIOS_OK;
     }
     DirectArgs da{};
@@ -467,6 +488,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
 #undef HELIOS_DIRECT_CASE
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
+    stamp(c, 2);
     return HELIOS_OK;
 }
 
@@ -489,7 +511,9 @@ int helios_forward_highres(helios_ctx* c, int B, const double* params, float* fl
     CU_TRY(c, cudaSetDevice(c->device));
     if ((rc = helios_reserve(c, B))) return rc;
     c->n_models += B;
-    return run_flux(c, B, params, flux_out, c->nNu);
+    rc = run_flux(c, B, params, flux_out, c->nNu);
+    if (c->opt_timing) { c->ev_has_obs[c->timed_calls % helios_ctx::kTimingRing] = false; c->timed_calls++; }
+    return rc;
 }
 
 int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spectra_out, double* logl_out) {
@@ -507,6 +531,8 @@ int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spec
     k_obs_apply<<<B, kObsThreads, 0, c->stream>>>(oa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
+    stamp(c, 3);
+    if (c->opt_timing) { c->ev_has_obs[c->timed_calls % helios_ctx::kTimingRing] = true; c->timed_calls++; }
     return HELIOS_OK;
 }
 
@@ -531,6 +557,24 @@ int helios_forward_batch_host(helios_ctx* c, int B, const double* params_host, f
     if (logl_host)
         CU_TRY(c, cudaMemcpyAsync(logl_host, c->d_logl_stage, sizeof(double) * B, cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return HELIOS_OK;
+}
+
+int helios_get_stage_ms(helios_ctx* c, double* stage_ms, int* n_calls) {
+    if (!c || !stage_ms || !n_calls) return HELIOS_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    const int n = (int)std::min<long long>(c->timed_calls, helios_ctx::kTimingRing);
+    double acc[3] = {0, 0, 0};
+    int n_obs = 0;
+    for (int i = 0; i < n; ++i) {
+        float ms = 0;
+        CU_TRY(c, cudaEventElapsedTime(&ms, c->ev[i][0], c->ev[i][1])); acc[0] += ms;
+        CU_TRY(c, cudaEventElapsedTime(&ms, c->ev[i][1], c->ev[i][2])); acc[1] += ms;
+        if (c->ev_has_obs[i]) { CU_TRY(c, cudaEventElapsedTime(&ms, c->ev[i][2], c->ev[i][3])); acc[2] += ms; ++n_obs; }
+    }
+    stage_ms[0] = n ? acc[0] / n : 0; stage_ms[1] = n ? acc[1] / n : 0; stage_ms[2] = n_obs ? acc[2] / n_obs : 0;
+    *n_calls = n;
     return HELIOS_OK;
 }
 

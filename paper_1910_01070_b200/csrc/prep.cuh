@@ -99,7 +99,12 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
         rec[o++] = (float)(w * t);
     }
     // Planck exponent scale and half layer thickness (hydrostatic, ideal gas; R5)
-    rec[o++] = (float)(kC2 * kLog2e / T);
+    {
+        const double a = kC2 * kLog2e / T;
+        const float a_hi = (float)a;
+        rec[o++] = a_hi;
+        rec[o++] = (float)(a - (double)a_hi);
+    }
     double hdz = 0.0;
     if (l + 1 < a.L) {
         double T_up = knot_temperature(knots, a.K, a.lvl_knot[l + 1], a.lvl_xi[l + 1]);
@@ -112,7 +117,6 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
         rec[o++] = __int_as_float(iT);
     } else {
         rec[o++] = __int_as_float(iT);
-        rec[o++] = 0.0f;
     }
     while (o < a.rec_floats) rec[o++] = 0.0f;
 }

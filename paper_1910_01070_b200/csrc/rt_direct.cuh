@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
 
     const double nu_d = a.nu0 + a.dnu * (double)inu;
     const float nu = (float)nu_d;
+    const float nu_lo = (float)(nu_d - (double)nu);
     const float c1nu3 = (float)(kC1 * nu_d * nu_d * nu_d);
     const int PA = 4 * a.S + 2 * a.C;
     const long long plane = (long long)a.nT * a.nP * a.stride;
@@ -53,8 +54,8 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
 
     for (int l = 0; l < a.L; ++l) {
         const float* r = srec + l * a.rec_floats;
-        const int cell = __float_as_int(r[PA + 2]);
-        const int iT = __float_as_int(r[PA + 3]);
+        const int cell = __float_as_int(r[PA + 3]);
+        const int iT = __float_as_int(r[PA + 4]);
         float chi = 0.0f;
         const float* tab = a.sigma + (long long)cell * a.stride + inu;
         for (int s = 0; s < a.S; ++s) {
@@ -71,8 +72,8 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
             chi = fmaf(r[4 * a.S + 2 * c + 1], __ldg(a0 + a.stride), chi);
         }
         // S_l = B_nu(T_l) = c1 nu^3 E / (1 - E), E = exp(-c2 nu / T_l)
-        const float E = ex2_approx(-r[PA] * nu);
-        const float Sl = c1nu3 * __fdividef(E, 1.0f - E);
+        const float E = planck_E(r[PA], r[PA + 1], nu, nu_lo);
+        const float Sl = planck_from_E(c1nu3, E);
         if (l > 0) {
             const float dtau = (chi + chi_prev) * hdz_prev;
             const float inv_dtau = rcp_approx(dtau);
@@ -81,7 +82,7 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
             for (int k = 0; k < A; ++k)
                 sc_update(J[k], dtau, inv_dtau, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
         }
-        chi_prev = chi; S_prev = Sl; hdz_prev = r[PA + 1];
+        chi_prev = chi; S_prev = Sl; hdz_prev = r[PA + 2];
     }
     // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = J_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
     float acc = S_prev * a.ang.wmu_sum;
