@@ -33,10 +33,17 @@ constexpr int kMaxCia = 2;
 //   +4  iT                               (int bits)
 __host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S + 2 * C + 5 + 3) & ~3; }
 
-// Slab kernel record, fp32 (p-blend is shared by all models, so 2 taps per row):
-//   [0, 2R)  pairs {a_r, b_r}: weights of the p-blended rows iT and iT+1, r < R = S + C
-//   +0 planck_a (high)  +1 planck_a (low)  +2 hdz  +3 iT (int bits)
-__host__ __device__ inline int slab_rec_floats(int R) { return (2 * R + 4 + 3) & ~3; }
+// Staged ("slab") kernel, fp32.  VMRs are constant with height, so the species
+// sum commutes with the bilinear blend: chi_l = sum_corners w_corner G_corner with
+// G_corner(nu) = sum_s x_s sigma_s[corner](nu), recomputed only when the model leaves a table cell.
+// Per-(model, level) record, kSlabRecFloats floats:
+//   0..3  n 2^-32 {(1-t)(1-u), (1-t)u, t(1-u), t u}   weights of G at (iT,ip), (iT,ip+1), (iT+1,ip), (iT+1,ip+1)
+//   4..5  am^2 {(1-t), t}                               weights of the CIA mix at iT, iT+1
+//   6..7  planck_a high / low      8  hdz      9  iT (int bits)      10..11  unused
+// Per-model vector, slab_x_floats(S, C) floats: x_s 2^32 (S values), then x_H2 x_c (C values).
+constexpr int kSlabRecFloats = 12;
+constexpr float kSlabXScale = 4294967296.0f;   // 2^32: keeps x_s sigma_s far above the fp32 denormal range
+__host__ __device__ inline int slab_x_floats(int S, int C) { return (S + C + 3) & ~3; }
 
 struct AngleSet {
     int   n;
@@ -79,28 +86,29 @@ __device__ __forceinline__ float planck_from_E(float c1nu3, float E) {
 // Short-characteristics update for one angle in deviation form.
 // With J = I - S(level) and dS = S_{l-1} - S_l, Eq. 4-6 read
 //   J_l = e^{-D} J_{l-1} + phi(D) dS,   phi(D) = (1 - e^{-D})/D,   D = dtau / mu  (Eq. 7)
-// (beta = 1 - phi, gamma = phi - e^{-D}).  phi is evaluated by its Taylor series for
-// D < kPhiSwitch, where (1 - e^{-D})/D cancels in fp32 (R10).
+// (beta = 1 - phi, gamma = phi - e^{-D}).  For D < kPhiSwitch, where (1 - e^{-D})/D cancels
+// in fp32, phi comes from a degree-4 near-minimax polynomial (R10).
 constexpr float kPhiSwitch = 0.25f;
-__device__ __forceinline__ float phi_series(float D) {
-    // 1 - D/2 + D^2/6 - D^3/24 + D^4/120 - D^5/720 + D^6/5040   (|error| < 7e-9 for D < 1/4)
-    float p = fmaf(D, 1.0f / 5040.0f, -1.0f / 720.0f);
-    p = fmaf(D, p, 1.0f / 120.0f);
-    p = fmaf(D, p, -1.0f / 24.0f);
-    p = fmaf(D, p, 1.0f / 6.0f);
-    p = fmaf(D, p, -0.5f);
+__device__ __forceinline__ float phi_small(float D) {
+    // Chebyshev-node interpolant of (1 - e^{-D})/D on [0, 1/4]; |error| < 5e-9 with these
+    // fp32 coefficients (Taylor would need degree 6 for the same bound).
+    float p = fmaf(D, 0x1.ec6964p-8f, -0x1.53e436p-5f);
+    p = fmaf(D, p, 0x1.554d2ap-3f);
+    p = fmaf(D, p, -0x1.ffffe0p-2f);
     return fmaf(D, p, 1.0f);
 }
-// Small D: e^{-D} = 1 - D phi(D) exactly, so J_l = J + phi (dS - D J): two correctly rounded
+// Small D: e^{-D} = 1 - D phi(D) exactly, so J_l = J + phi (dS - D J): correctly rounded
 // FMAs and no exponential.  (MUFU.EX2 results just below 1 carry a one-sided error of a
 // fraction of an ulp; through ~50 transparent layers that biased the flux by -4e-7, which
-// the absolute logL tolerance does not allow.)  Large D: hardware 2^x.
-__device__ __forceinline__ void sc_update(float& J, float dtau, float inv_dtau, float dS,
+// the absolute logL tolerance does not allow.)  Large D: hardware 2^x, J_l = e J + (1 - e) t
+// with t = mu dS / dtau.  q = dS / dtau is shared by all angles of the layer.
+__device__ __forceinline__ void sc_update(float& J, float dtau, float q, float dS,
                                           float c_exp, float inv_mu, float mu) {
     const float D = dtau * inv_mu;
     const float e = ex2_approx(-dtau * c_exp);
-    const float J_big = fmaf(e, J, (1.0f - e) * (mu * inv_dtau) * dS);
-    const float J_small = fmaf(phi_series(D), fmaf(-D, J, dS), J);
+    const float t = mu * q;
+    const float J_big = fmaf(e, J, fmaf(-e, t, t));
+    const float J_small = fmaf(phi_small(D), fmaf(-D, J, dS), J);
     J = (D < kPhiSwitch) ? J_small : J_big;
 }
 

@@ -45,8 +45,13 @@ struct helios_ctx {
     double* d_lvl_p = nullptr; int* d_lvl_knot = nullptr; double* d_lvl_xi = nullptr;
     int* d_lvl_ip = nullptr; double* d_lvl_u = nullptr; int* d_lvl_pclamp = nullptr;
     double* d_lvl_lnratio = nullptr;
-    float* d_lvl_uf = nullptr;          // [L] fp32 pressure weight (slab kernel)
     std::vector<int> lvl_ip;
+    // staged kernel: plane schedule (segments of constant pressure cell) and TMA views of the tables
+    int n_seg = 0, n_loads = 0;
+    int* d_seg_lbegin = nullptr; int* d_seg_hi = nullptr; int* d_seg_lo = nullptr; int* d_load_ip = nullptr;
+    bool have_tmaps = false;
+    CUtensorMap tm_sigma{}, tm_cia{};
+    size_t smem_optin = 0, smem_sm = 0;
 
     // ---- observation
     bool have_obs = false, have_data = false;
@@ -59,7 +64,7 @@ struct helios_ctx {
     int cap_B = 0;
     float* d_rec = nullptr; size_t rec_bytes = 0;
     float* d_flux = nullptr; long long flux_stride = 0;
-    float* d_scale = nullptr; int* d_flag = nullptr;
+    float* d_scale = nullptr; int* d_flag = nullptr; float* d_model_x = nullptr;
     unsigned long long* d_counters = nullptr;    // [2]
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
@@ -109,10 +114,54 @@ static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
 static void free_all(helios_ctx* c) {
     dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid);
     dfree(c->d_lvl_p); dfree(c->d_lvl_knot); dfree(c->d_lvl_xi); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
-    dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio); dfree(c->d_lvl_uf);
+    dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
+    dfree(c->d_seg_lbegin); dfree(c->d_seg_hi); dfree(c->d_seg_lo); dfree(c->d_load_ip);
     dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
-    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_counters);
+    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x); dfree(c->d_counters);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
+}
+
+// TMA views of the resident tables for the staged kernel (cuTensorMapEncodeTiled, resolved through
+// the runtime so that libcuda is not a link-time dependency):
+//   sigma {nu (padded row), ip, iT, s}, box {32, 1, nT, 1};   cia {nu, iT, c}, box {32, nT, 1}.
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static bool build_tensor_maps(helios_ctx* c) {
+    c->have_tmaps = false;
+    std::memset(&c->tm_sigma, 0, sizeof c->tm_sigma);
+    std::memset(&c->tm_cia, 0, sizeof c->tm_cia);
+    if (c->nT > 256) return false;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
+        qres != cudaDriverEntryPointSuccess || !fn) {
+        cudaGetLastError();
+        return false;
+    }
+    encode_tiled_fn encode = (encode_tiled_fn)fn;
+    const cuuint64_t row = (cuuint64_t)c->stride * sizeof(float);
+    if (c->S > 0) {
+        cuuint64_t dims[4] = {(cuuint64_t)c->stride, (cuuint64_t)c->nP, (cuuint64_t)c->nT, (cuuint64_t)c->S};
+        cuuint64_t strides[3] = {row, row * c->nP, row * c->nP * c->nT};
+        cuuint32_t box[4] = {(cuuint32_t)kSlabTile, 1, (cuuint32_t)c->nT, 1};
+        cuuint32_t estr[4] = {1, 1, 1, 1};
+        if (encode(&c->tm_sigma, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->d_sigma, dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
+    }
+    if (c->C > 0) {
+        cuuint64_t dims[3] = {(cuuint64_t)c->stride, (cuuint64_t)c->nT, (cuuint64_t)c->C};
+        cuuint64_t strides[2] = {row, row * c->nT};
+        cuuint32_t box[3] = {(cuuint32_t)kSlabTile, (cuuint32_t)c->nT, 1};
+        cuuint32_t estr[3] = {1, 1, 1};
+        if (encode(&c->tm_cia, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->d_cia, dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
+    }
+    c->have_tmaps = true;
+    return true;
 }
 
 extern "C" {
@@ -138,6 +187,9 @@ int helios_create(helios_ctx** out, int device, void* cuda_stream) {
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, device);
+    int v = 0;
+    cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device); c->smem_optin = (size_t)v;
+    cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device); c->smem_sm = (size_t)v;
     e = cudaMalloc(&c->d_counters, 2 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, 2 * sizeof(unsigned long long));
     if (e != cudaSuccess) { delete c; return fail(nullptr, HELIOS_ECUDA, "helios_create: %s", cudaGetErrorString(e)); }
@@ -169,7 +221,8 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value < 0 || value > 2) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1 or 2");
             c->opt_kernel = value; return HELIOS_OK;
         case HELIOS_OPT_MODELS_PER_CTA:
-            if (value < 0) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be >= 0");
+            if (value != 0 && value != 8 && value != 12 && value != 16)
+                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 12 or 16");
             c->opt_models_per_cta = value; return HELIOS_OK;
         case HELIOS_OPT_TIMING:
             c->opt_timing = value ? 1 : 0; c->timed_calls = 0;
@@ -219,6 +272,7 @@ int helios_load_opacity(helios_ctx* c, int S, int nT, const double* T_grid, int 
     }
     CU_TRY(c, upload(c->d_Tgrid, c->T_grid, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    build_tensor_maps(c);      // failure only disables the staged kernel
     c->have_tables = true;
     c->cap_B = 0;    // record size depends on S, C
     return HELIOS_OK;
@@ -275,7 +329,6 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
 
     std::vector<double> p(L), xi(L), u(L), lnr(L, 0.0);
     std::vector<int> knot(L), ip(L), pcl(L);
-    std::vector<float> uf(L);
     const double x_bot = std::log10(p_bot), x_top = std::log10(p_top);
     for (int l = 0; l < L; ++l) {
         p[l] = p_bot * std::pow(p_top / p_bot, (double)l / (double)(L - 1));   // equidistant in log p
@@ -286,7 +339,6 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
         if (k > K - 2) k = K - 2 < 0 ? 0 : K - 2;
         knot[l] = k; xi[l] = s - k;
         axis_cell(c->lp_grid, x, ip[l], u[l], pcl[l]);
-        uf[l] = (float)u[l];
     }
     for (int l = 0; l + 1 < L; ++l) lnr[l] = std::log(p[l] / p[l + 1]);
     c->lvl_ip = ip;
@@ -297,7 +349,32 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
     CU_TRY(c, upload(c->d_lvl_u, u, c->stream));
     CU_TRY(c, upload(c->d_lvl_pclamp, pcl, c->stream));
     CU_TRY(c, upload(c->d_lvl_lnratio, lnr, c->stream));
-    CU_TRY(c, upload(c->d_lvl_uf, uf, c->stream));
+
+    // plane schedule of the staged kernel: segments of constant pressure cell; segment k needs the
+    // table planes ip_k + 1 ("hi") and ip_k ("lo"); a plane already loaded for the previous
+    // segment is reused, so with levels denser than table nodes there is one new load per segment.
+    {
+        std::vector<int> seg_lbegin, seg_hi, seg_lo, load_ip;
+        for (int l = 0; l < L; ++l) {
+            if (l > 0 && ip[l] == ip[l - 1]) continue;
+            seg_lbegin.push_back(l);
+            auto find_or_load = [&](int node) {
+                const int n = (int)load_ip.size();
+                for (int e = std::max(0, n - 2); e < n; ++e) if (load_ip[e] == node) return e;
+                load_ip.push_back(node);
+                return n;
+            };
+            const int hi = find_or_load(ip[l] + 1);
+            const int lo = find_or_load(ip[l]);
+            seg_hi.push_back(hi); seg_lo.push_back(lo);
+        }
+        seg_lbegin.push_back(L);
+        c->n_seg = (int)seg_hi.size(); c->n_loads = (int)load_ip.size();
+        CU_TRY(c, upload(c->d_seg_lbegin, seg_lbegin, c->stream));
+        CU_TRY(c, upload(c->d_seg_hi, seg_hi, c->stream));
+        CU_TRY(c, upload(c->d_seg_lo, seg_lo, c->stream));
+        CU_TRY(c, upload(c->d_load_ip, load_ip, c->stream));
+    }
 
     std::vector<double> x, W;
     gauss_legendre(A, x, W);
@@ -406,10 +483,11 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
     return HELIOS_OK;
 }
 
-static int use_slab(const helios_ctx* c, int B) {
-    if (c->opt_kernel == 1) return 0;
-    if (c->opt_kernel == 2) return 1;
-    return slab_supported(c->S, c->C, c->nT, c->A) && B >= 16;
+static SlabPlan plan_slab(const helios_ctx* c, int B) {
+    SlabPlan none;
+    if (c->opt_kernel == 1 || !c->have_tmaps) return none;
+    if (c->opt_kernel == 0 && B < 8) return none;      // a few models: the direct kernel streams the table once
+    return slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, c->opt_models_per_cta, c->smem_optin, c->smem_sm);
 }
 
 int helios_reserve(helios_ctx* c, int B) {
@@ -419,15 +497,16 @@ int helios_reserve(helios_ctx* c, int B) {
     if (B <= c->cap_B) return HELIOS_OK;
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
-    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag);
+    dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
     c->cap_B = 0;
-    const int rf = std::max(direct_rec_floats(c->S, c->C), slab_rec_floats(c->S + c->C));
+    const int rf = std::max(direct_rec_floats(c->S, c->C), kSlabRecFloats);
     c->flux_stride = c->stride;
     CU_TRY(c, cudaMalloc(&c->d_rec, sizeof(float) * (size_t)B * c->L * rf));
     CU_TRY(c, cudaMalloc(&c->d_flux, sizeof(float) * (size_t)B * c->flux_stride));
     CU_TRY(c, cudaMalloc(&c->d_scale, sizeof(float) * B));
     CU_TRY(c, cudaMalloc(&c->d_flag, sizeof(int) * B));
+    CU_TRY(c, cudaMalloc(&c->d_model_x, sizeof(float) * (size_t)B * slab_x_floats(c->S, c->C)));
     CU_TRY(c, cudaMalloc(&c->d_params_stage, sizeof(double) * (size_t)B * (2 + c->K + c->S)));
     CU_TRY(c, cudaMalloc(&c->d_spectra_stage, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
     CU_TRY(c, cudaMalloc(&c->d_logl_stage, sizeof(double) * B));
@@ -441,14 +520,18 @@ static inline void stamp(helios_ctx* c, int which) {
 
 // steps 0-4: params -> flux (DEVICE [B][flux_stride])
 static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride) {
-    const int slab = use_slab(c, B);
-    const int rf = slab ? slab_rec_floats(c->S + c->C) : direct_rec_floats(c->S, c->C);
+    const SlabPlan plan = plan_slab(c, B);
+    if (c->opt_kernel == 2 && !plan.ok)
+        return fail(c, HELIOS_EINVAL, "staged kernel requested but unavailable for this table shape (shared memory / TMA)");
+    const int slab = plan.ok ? 1 : 0;
+    const int rf = slab ? kSlabRecFloats : direct_rec_floats(c->S, c->C);
     PrepArgs pa{};
     pa.params = params; pa.B = B; pa.P = 2 + c->K + c->S; pa.K = c->K; pa.S = c->S; pa.C = c->C; pa.L = c->L;
     pa.nT = c->nT; pa.nP = c->nP; pa.T_grid = c->d_Tgrid; pa.lvl_p_bar = c->d_lvl_p; pa.lvl_knot = c->d_lvl_knot;
     pa.lvl_xi = c->d_lvl_xi; pa.lvl_ip = c->d_lvl_ip; pa.lvl_u = c->d_lvl_u; pa.lvl_pclamp = c->d_lvl_pclamp;
     pa.lvl_lnratio = c->d_lvl_lnratio; pa.mmw = c->mmw; pa.he_to_h2 = c->he_to_h2; pa.flux_const = c->flux_const;
     pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
+    pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
     pa.counters = c->d_counters;
     stamp(c, 0);
     k_prep<<<(B * c->L + 127) / 128, 128, 0, c->stream>>>(pa);
@@ -458,14 +541,15 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
 
     if (slab) {
         SlabArgs sa{};
-        sa.sigma = c->d_sigma; sa.cia = c->d_cia; sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nP = c->nP; sa.nNu = c->nNu;
-        sa.L = c->L; sa.B = B; sa.stride = c->stride; sa.lvl_ip = c->d_lvl_ip; sa.lvl_u = c->d_lvl_uf; sa.rec = c->d_rec;
-        sa.rec_floats = rf; sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu;
-        sa.flux = flux; sa.flux_stride = flux_stride; sa.ang = c->ang;
-        int nl = 0;
-        cudaError_t e = launch_rt_slab(sa, c->A, c->opt_models_per_cta, c->num_sms, c->stream, &nl);
-        c->n_launches += nl;
-        if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "slab kernel launch failed: %s", cudaGetErrorString(e));
+        sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nNu = c->nNu; sa.L = c->L; sa.B = B;
+        sa.rec = c->d_rec; sa.model_x = c->d_model_x; sa.x_floats = pa.x_floats;
+        sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu;
+        sa.flux = flux; sa.flux_stride = flux_stride;
+        sa.seg_lbegin = c->d_seg_lbegin; sa.seg_hi = c->d_seg_hi; sa.seg_lo = c->d_seg_lo; sa.load_ip = c->d_load_ip;
+        sa.n_seg = c->n_seg; sa.n_loads = c->n_loads; sa.ring = plan.ring; sa.ang = c->ang;
+        cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->stream);
+        if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "staged kernel launch failed: %s", cudaGetErrorString(e));
+        c->n_launches += 1;
         stamp(c, 2);
         return HELIOS_OK;
     }

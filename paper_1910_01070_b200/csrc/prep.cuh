@@ -21,7 +21,9 @@ struct PrepArgs {
     double mmw, he_to_h2, flux_const;
     float* rec;               // DEVICE [B][L][rec_floats]
     int rec_floats;
-    int slab_layout;          // 0: direct (4 taps / species), 1: slab (2 taps / row)
+    int slab_layout;          // 0: direct record (4 taps / species), 1: staged-kernel record (common.cuh)
+    float* model_x;           // DEVICE [B][x_floats]  staged kernel: x_s 2^32, x_H2 x_c
+    int x_floats;
     float* model_scale;       // DEVICE [B]  f * flux_const * 2 pi
     int*   model_flag;        // DEVICE [B]  1 = non-finite parameter
     unsigned long long* counters;  // [0] clamped pairs, [1] non-finite models
@@ -48,6 +50,7 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     }
     if (!finite) {
         for (int i = 0; i < a.rec_floats; ++i) rec[i] = 0.0f;
+        if (l == 0 && a.slab_layout) for (int i = 0; i < a.x_floats; ++i) a.model_x[(size_t)b * a.x_floats + i] = 0.0f;
         return;
     }
 
@@ -86,17 +89,26 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
             rec[o++] = (float)(w * t * (1.0 - u));
             rec[o++] = (float)(w * t * u);
         }
-    } else {
-        for (int s = 0; s < a.S; ++s) {
-            double w = n * pow(10.0, lvmr[s]);
+        for (int c = 0; c < a.C; ++c) {
+            double w = am * am * x_h2 * (c == 0 ? x_h2 : x_he);
             rec[o++] = (float)(w * (1.0 - t));
             rec[o++] = (float)(w * t);
         }
-    }
-    for (int c = 0; c < a.C; ++c) {
-        double w = am * am * x_h2 * (c == 0 ? x_h2 : x_he);
-        rec[o++] = (float)(w * (1.0 - t));
-        rec[o++] = (float)(w * t);
+    } else {
+        const double w = n / (double)kSlabXScale;
+        rec[o++] = (float)(w * (1.0 - t) * (1.0 - u));
+        rec[o++] = (float)(w * (1.0 - t) * u);
+        rec[o++] = (float)(w * t * (1.0 - u));
+        rec[o++] = (float)(w * t * u);
+        rec[o++] = (float)(am * am * (1.0 - t));
+        rec[o++] = (float)(am * am * t);
+        if (l == 0) {
+            float* mx = a.model_x + (size_t)b * a.x_floats;
+            int k = 0;
+            for (int s = 0; s < a.S; ++s) mx[k++] = (float)(pow(10.0, lvmr[s]) * (double)kSlabXScale);
+            for (int c = 0; c < a.C; ++c) mx[k++] = (float)(x_h2 * (c == 0 ? x_h2 : x_he));
+            while (k < a.x_floats) mx[k++] = 0.0f;
+        }
     }
     // Planck exponent scale and half layer thickness (hydrostatic, ideal gas; R5)
     {
@@ -112,12 +124,8 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
         hdz = 0.5 * dz;
     }
     rec[o++] = (float)hdz;
-    if (!a.slab_layout) {
-        rec[o++] = __int_as_float(iT * a.nP + a.lvl_ip[l]);
-        rec[o++] = __int_as_float(iT);
-    } else {
-        rec[o++] = __int_as_float(iT);
-    }
+    if (!a.slab_layout) rec[o++] = __int_as_float(iT * a.nP + a.lvl_ip[l]);
+    rec[o++] = __int_as_float(iT);
     while (o < a.rec_floats) rec[o++] = 0.0f;
 }
 

@@ -76,11 +76,11 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
         const float Sl = planck_from_E(c1nu3, E);
         if (l > 0) {
             const float dtau = (chi + chi_prev) * hdz_prev;
-            const float inv_dtau = rcp_approx(dtau);
             const float dS = S_prev - Sl;
+            const float q = dS * rcp_approx(dtau);
 #pragma unroll
             for (int k = 0; k < A; ++k)
-                sc_update(J[k], dtau, inv_dtau, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
+                sc_update(J[k], dtau, q, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
         }
         chi_prev = chi; S_prev = Sl; hdz_prev = r[PA + 2];
     }

@@ -1,22 +1,308 @@
-// rt_slab.cuh -- large-batch variant of fused steps 1-4 (placeholder until the staged kernel lands)
+// rt_slab.cuh -- fused steps 1-4, large-batch variant.
+//
+// One CTA = NW compute warps + 1 producer warp, working on ONE 32-point wavenumber tile
+// for NW models (compute warp w = model w of the group, lane = wavenumber).
+//
+// Table staging.  The levels are a fixed log-p grid, so the pressure cell of
+// level l is the same for every model.  Levels are grouped into SEGMENTS of constant pressure
+// cell; a segment needs two PLANES of the table, plane(ip) = sigma[all s][all iT][ip][tile]
+// (S*nT rows of 128 B).  The producer thread streams the planes through a ring of NB shared
+// memory slots with TMA (cp.async.bulk.tensor.4d, one box per species, mbarrier completion);
+// consumers release a slot through an "empty" mbarrier when they leave the last segment that
+// needs it.  Every table row is therefore read from L2 once per CTA and reused by all NW
+// models and all levels of the segment; rows of the CIA tables are staged once.
+//
+// Cell walk.  VMRs are constant with height, so with G_c = sum_s x_s sigma_s at
+// the four corners c of the model's current (T, p) cell, chi_l = n_l sum_c b_c G_c (b = bilinear
+// weights): the species sum is redone only when the model enters another cell (every ~5 levels),
+// not at every level.  Algebraically identical to interpolating each species and then summing
+// (PAPER.md:241, 127); only the fp32 summation order differs.
+//
+// RT, Planck, optical depth: as in rt_direct.cuh (Eq. 2, 4-9), state in registers.
 #pragma once
+#include <cuda.h>
+
 #include "common.cuh"
 
 namespace helios {
 
+constexpr int kSlabTile = 32;       // wavenumbers per CTA (one 128 B row segment per table row)
+constexpr int kSlabMaxRing = 8;
+
 struct SlabArgs {
-    const float* sigma; const float* cia;
-    int S, C, nT, nP, nNu, L, B;
-    long long stride;
-    const int* lvl_ip; const float* lvl_u;
-    const float* rec; int rec_floats;
-    const float* model_scale; const int* model_flag;
+    int S, C, nT, nNu, L, B;
+    const float* rec;               // DEVICE [B][L][kSlabRecFloats]
+    const float* model_x;           // DEVICE [B][x_floats]
+    int x_floats;
+    const float* model_scale;
+    const int* model_flag;
     double nu0, dnu;
-    float* flux; long long flux_stride;
+    float* flux;                    // DEVICE [B][flux_stride]
+    long long flux_stride;
+    // plane schedule (helios_set_atmosphere)
+    const int* seg_lbegin;          // DEVICE [n_seg + 1] first level of each segment
+    const int* seg_hi;              // DEVICE [n_seg] load index holding plane ip+1
+    const int* seg_lo;              // DEVICE [n_seg] load index holding plane ip
+    const int* load_ip;             // DEVICE [n_loads] pressure node of each load, in issue order
+    int n_seg, n_loads;
+    int ring;                       // NB, number of plane slots
     AngleSet ang;
 };
 
-inline bool slab_supported(int, int, int, int) { return false; }
-inline cudaError_t launch_rt_slab(const SlabArgs&, int, int, int, cudaStream_t, int*) { return cudaErrorNotSupported; }
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA: one box of the 4-D table view {nu, ip, iT, s} / the 3-D CIA view {nu, iT, c} -> shared memory
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+// shared memory: [ring][S*nT*32] planes | [C*nT*32] CIA | [NW][x_floats] | mbarriers
+__host__ __device__ inline size_t slab_plane_floats(int S, int nT) { return (size_t)S * nT * kSlabTile; }
+__host__ __device__ inline size_t slab_fixed_bytes(int C, int nT, int NW, int x_floats) {
+    return sizeof(float) * ((size_t)C * nT * kSlabTile + (size_t)NW * x_floats) + 8 * (2 * kSlabMaxRing + 1) + 128;
+}
+
+template <int A, int NW, int MINB>
+__global__ void __launch_bounds__((NW + 1) * 32, MINB)
+k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ CUtensorMap tm_cia, SlabArgs a) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const size_t plane_floats = slab_plane_floats(a.S, a.nT);
+    float* planes = reinterpret_cast<float*>(smem_raw);
+    float* cia_s = planes + (size_t)a.ring * plane_floats;
+    float* xs_s = cia_s + (size_t)a.C * a.nT * kSlabTile;
+    uint64_t* full = reinterpret_cast<uint64_t*>(xs_s + NW * a.x_floats);
+    uint64_t* empty = full + kSlabMaxRing;
+    uint64_t* cia_bar = empty + kSlabMaxRing;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = blockIdx.y, group = blockIdx.x;
+    const int NB = a.ring;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NB; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NW); }
+        mbar_init(cia_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == NW) {
+        // ===== producer: stream the planes this tile needs, in schedule order =====
+        if (lane == 0) {
+            const int nu_first = tile * kSlabTile;
+            if (a.C > 0) {
+                mbar_expect_tx(cia_bar, (uint32_t)(sizeof(float) * a.C * a.nT * kSlabTile));
+                for (int c = 0; c < a.C; ++c)
+                    tma_load_3d(cia_s + (size_t)c * a.nT * kSlabTile, &tm_cia, cia_bar, nu_first, 0, c);
+            }
+            if (a.S > 0) {
+                for (int e = 0; e < a.n_loads; ++e) {
+                    const int slot = e % NB, use = e / NB;
+                    if (use > 0) mbar_wait(&empty[slot], (uint32_t)((use - 1) & 1));
+                    const int ip = a.load_ip[e];
+                    float* dst = planes + (size_t)slot * plane_floats;
+                    mbar_expect_tx(&full[slot], (uint32_t)(sizeof(float) * plane_floats));
+                    for (int s = 0; s < a.S; ++s)
+                        tma_load_4d(dst + (size_t)s * a.nT * kSlabTile, &tm_sigma, &full[slot], nu_first, ip, 0, s);
+                }
+            }
+        }
+        return;
+    }
+
+    // ===== consumers: warp = model, lane = wavenumber =====
+    int b = group * NW + warp;
+    const bool model_valid = b < a.B;
+    if (!model_valid) b = a.B - 1;           // still takes part in the slot hand-shake
+    float* xw = xs_s + warp * a.x_floats;
+    for (int i = lane; i < a.x_floats; i += 32) xw[i] = a.model_x[(size_t)b * a.x_floats + i];
+    __syncwarp();
+
+    const int inu = tile * kSlabTile + lane;
+    const double nu_d = a.nu0 + a.dnu * (double)inu;
+    const float nu = (float)nu_d;
+    const float nu_lo = (float)(nu_d - (double)nu);
+    const float c1nu3 = (float)(kC1 * nu_d * nu_d * nu_d);
+    const int row = a.nT * kSlabTile;         // floats between species in a plane
+    const float4* rec4 = reinterpret_cast<const float4*>(a.rec + (size_t)b * a.L * kSlabRecFloats);
+
+    float J[A];
+#pragma unroll
+    for (int k = 0; k < A; ++k) J[k] = 0.0f;
+    float chi_prev = 0.0f, S_prev = 0.0f, hdz_prev = 0.0f;
+    float G00 = 0.0f, G01 = 0.0f, G10 = 0.0f, G11 = 0.0f, Gc0 = 0.0f, Gc1 = 0.0f;
+    int released = 0;
+
+    if (a.C > 0) mbar_wait(cia_bar, 0);
+
+    for (int seg = 0; seg < a.n_seg; ++seg) {
+        const int l_begin = a.seg_lbegin[seg], l_end = a.seg_lbegin[seg + 1];
+        const float* pLo = planes + lane;
+        const float* pHi = planes + lane;
+        if (a.S > 0) {
+            const int eHi = a.seg_hi[seg], eLo = a.seg_lo[seg];
+            mbar_wait(&full[eHi % NB], (uint32_t)((eHi / NB) & 1));
+            mbar_wait(&full[eLo % NB], (uint32_t)((eLo / NB) & 1));
+            pHi += (size_t)(eHi % NB) * plane_floats;
+            pLo += (size_t)(eLo % NB) * plane_floats;
+        }
+        int cur_iT = -1;
+        for (int l = l_begin; l < l_end; ++l) {
+            const float4 r0 = __ldg(rec4 + 3 * l), r1 = __ldg(rec4 + 3 * l + 1), r2 = __ldg(rec4 + 3 * l + 2);
+            const int iT = __float_as_int(r2.y);
+            if (iT != cur_iT) {               // warp-uniform: the model entered another table cell
+                cur_iT = iT;
+                const float* qLo = pLo + iT * kSlabTile;
+                const float* qHi = pHi + iT * kSlabTile;
+                G00 = G01 = G10 = G11 = 0.0f;
+                for (int s = 0; s < a.S; ++s) {
+                    const float x = xw[s];
+                    G00 = fmaf(x, qLo[s * row], G00);
+                    G10 = fmaf(x, qLo[s * row + kSlabTile], G10);
+                    G01 = fmaf(x, qHi[s * row], G01);
+                    G11 = fmaf(x, qHi[s * row + kSlabTile], G11);
+                }
+                Gc0 = Gc1 = 0.0f;
+                const float* qc = cia_s + iT * kSlabTile + lane;
+                for (int c = 0; c < a.C; ++c) {
+                    const float x = xw[a.S + c];
+                    Gc0 = fmaf(x, qc[c * row], Gc0);
+                    Gc1 = fmaf(x, qc[c * row + kSlabTile], Gc1);
+                }
+            }
+            float chi = r0.x * G00;
+            chi = fmaf(r0.y, G01, chi);
+            chi = fmaf(r0.z, G10, chi);
+            chi = fmaf(r0.w, G11, chi);
+            chi = fmaf(r1.x, Gc0, chi);
+            chi = fmaf(r1.y, Gc1, chi);
+            const float E = planck_E(r1.z, r1.w, nu, nu_lo);
+            const float Sl = planck_from_E(c1nu3, E);
+            if (l > 0) {
+                const float dtau = (chi + chi_prev) * hdz_prev;
+                const float dS = S_prev - Sl;
+                const float q = dS * rcp_approx(dtau);
+#pragma unroll
+                for (int k = 0; k < A; ++k)
+                    sc_update(J[k], dtau, q, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
+            }
+            chi_prev = chi; S_prev = Sl; hdz_prev = r2.x;
+        }
+        if (a.S > 0 && seg + 1 < a.n_seg) {
+            // slots holding loads older than the next segment's are free for the producer
+            const int next_first = min(a.seg_hi[seg + 1], a.seg_lo[seg + 1]);
+            __syncwarp();
+            if (lane == 0)
+                for (int e = released; e < next_first; ++e) mbar_arrive(&empty[e % NB]);
+            released = max(released, next_first);
+        }
+    }
+
+    if (!model_valid || inu >= a.nNu) return;
+    float* out = a.flux + (size_t)b * a.flux_stride + inu;
+    if (a.model_flag[b]) { *out = __int_as_float(0x7fc00000); return; }
+    // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = J_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
+    float acc = S_prev * a.ang.wmu_sum;
+#pragma unroll
+    for (int k = 0; k < A; ++k) acc = fmaf(a.ang.wmu[k], J[k], acc);
+    *out = a.model_scale[b] * acc;
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------
+struct SlabPlan {
+    bool ok = false;
+    int NW = 0, ring = 0;
+    size_t smem = 0;
+};
+
+// Picks the models-per-CTA variant and the ring depth that fit the shared memory of one SM.
+inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw, size_t smem_optin, size_t smem_sm) {
+    SlabPlan p;
+    if (A < 1 || A > kMaxAngles || nT > 256) return p;
+    const int nw = want_nw > 0 ? want_nw : 16;
+    if (nw != 8 && nw != 12 && nw != 16) return p;
+    const int target_ctas = nw == 8 ? 3 : 2;
+    const size_t plane = sizeof(float) * slab_plane_floats(S, nT);
+    const size_t fixed = slab_fixed_bytes(C, nT, nw, slab_x_floats(S, C));
+    for (int ctas = target_ctas; ctas >= 1; --ctas) {
+        size_t budget = smem_sm / ctas;
+        budget = budget > 1024 ? budget - 1024 : 0;     // per-CTA reservation of the runtime
+        if (budget > smem_optin) budget = smem_optin;
+        if (budget < fixed) continue;
+        int ring = plane ? (int)((budget - fixed) / plane) : 1;
+        if (ring > kSlabMaxRing) ring = kSlabMaxRing;
+        if (n_loads > 0 && ring > n_loads) ring = n_loads;
+        const int need = n_loads >= 3 ? 3 : (n_loads > 0 ? n_loads : 1);
+        if (plane && ring < need) continue;
+        if (ring < 1) ring = 1;
+        p.ok = true; p.NW = nw; p.ring = ring; p.smem = fixed + plane * ring;
+        return p;
+    }
+    return p;
+}
+
+template <int A, int NW, int MINB>
+inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, size_t smem,
+                                    cudaStream_t stream) {
+    cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const dim3 grid((a.B + NW - 1) / NW, (a.nNu + kSlabTile - 1) / kSlabTile);
+    k_rt_slab<A, NW, MINB><<<grid, (NW + 1) * 32, smem, stream>>>(tms, tmc, a);
+    return cudaGetLastError();
+}
+
+template <int A>
+inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
+                                    cudaStream_t stream) {
+    switch (p.NW) {
+        case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p.smem, stream);
+        case 12: return launch_rt_slab_t<A, 12, 2>(tms, tmc, a, p.smem, stream);
+        case 16: return launch_rt_slab_t<A, 16, 2>(tms, tmc, a, p.smem, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+inline cudaError_t launch_rt_slab(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
+                                  cudaStream_t stream) {
+    switch (a.ang.n) {
+        case 1: return launch_rt_slab_a<1>(tms, tmc, a, p, stream);
+        case 2: return launch_rt_slab_a<2>(tms, tmc, a, p, stream);
+        case 3: return launch_rt_slab_a<3>(tms, tmc, a, p, stream);
+        case 4: return launch_rt_slab_a<4>(tms, tmc, a, p, stream);
+        case 5: return launch_rt_slab_a<5>(tms, tmc, a, p, stream);
+        case 6: return launch_rt_slab_a<6>(tms, tmc, a, p, stream);
+        case 7: return launch_rt_slab_a<7>(tms, tmc, a, p, stream);
+        case 8: return launch_rt_slab_a<8>(tms, tmc, a, p, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
 
 }  // namespace helios
