@@ -52,7 +52,16 @@ struct AngleSet {
     float mu[kMaxAngles];
     float wmu[kMaxAngles];     // w_k mu_k
     float wmu_sum;             // sum_k w_k mu_k ( = 1/2 up to rounding)
+    // staged kernel, state H_k = J_k / mu_k (rt_slab.cuh)
+    float thr[kMaxAngles];     // kPhiSwitch * mu_k   : small-D branch iff dtau < thr
+    float pc[5][kMaxAngles];   // phi(dtau / mu_k) / mu_k = sum_j pc[j][k] dtau^j on the small-D branch
+    float wH[kMaxAngles];      // w_k mu_k^2
 };
+
+// Chebyshev-node interpolant of phi(D) = (1 - e^{-D})/D on [0, 1/4], degree 4 (|error| < 5e-9);
+// Taylor would need degree 6 for the same bound.  Constant term forced to 1.
+constexpr double kPhiC1 = -0.49999951482099264, kPhiC2 = 0.16665108206599635, kPhiC3 = -0.041490654102785796,
+                 kPhiC4 = 0.00751360621792363;
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
@@ -90,11 +99,9 @@ __device__ __forceinline__ float planck_from_E(float c1nu3, float E) {
 // in fp32, phi comes from a degree-4 near-minimax polynomial (R10).
 constexpr float kPhiSwitch = 0.25f;
 __device__ __forceinline__ float phi_small(float D) {
-    // Chebyshev-node interpolant of (1 - e^{-D})/D on [0, 1/4]; |error| < 5e-9 with these
-    // fp32 coefficients (Taylor would need degree 6 for the same bound).
-    float p = fmaf(D, 0x1.ec6964p-8f, -0x1.53e436p-5f);
-    p = fmaf(D, p, 0x1.554d2ap-3f);
-    p = fmaf(D, p, -0x1.ffffe0p-2f);
+    float p = fmaf(D, (float)kPhiC4, (float)kPhiC3);
+    p = fmaf(D, p, (float)kPhiC2);
+    p = fmaf(D, p, (float)kPhiC1);
     return fmaf(D, p, 1.0f);
 }
 // Small D: e^{-D} = 1 - D phi(D) exactly, so J_l = J + phi (dS - D J): correctly rounded

@@ -221,8 +221,8 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value < 0 || value > 2) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1 or 2");
             c->opt_kernel = value; return HELIOS_OK;
         case HELIOS_OPT_MODELS_PER_CTA:
-            if (value != 0 && value != 8 && value != 12 && value != 16)
-                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 12 or 16");
+            if (value != 0 && value != 8 && value != 16 && value != 24)
+                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16 or 24");
             c->opt_models_per_cta = value; return HELIOS_OK;
         case HELIOS_OPT_TIMING:
             c->opt_timing = value ? 1 : 0; c->timed_calls = 0;
@@ -251,7 +251,7 @@ int helios_load_opacity(helios_ctx* c, int S, int nT, const double* T_grid, int 
     c->have_tables = c->have_atmo = c->have_obs = c->have_data = false;
     dfree(c->d_sigma); dfree(c->d_cia);
     c->S = S; c->C = C; c->nT = nT; c->nP = nP; c->nNu = nNu; c->nu0 = nu0; c->dnu = dnu;
-    c->stride = ((long long)nNu + 31) / 32 * 32;
+    c->stride = ((long long)nNu + kSlabTile - 1) / kSlabTile * kSlabTile;   // rows padded to the staged kernel's tile (256 B)
     c->T_grid.assign(T_grid, T_grid + nT);
     c->lp_grid.assign(lp_grid, lp_grid + nP);
     const cudaMemcpyKind kind = (flags & HELIOS_PTRS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
@@ -390,6 +390,10 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
         g.inv_mu[k] = (float)(1.0 / c->mu[k]);
         g.c_exp[k] = (float)(kLog2e / c->mu[k]);
         g.wmu[k] = (float)(c->w[k] * c->mu[k]);
+        g.thr[k] = (float)(kPhiSwitch * c->mu[k]);
+        g.wH[k] = (float)(c->w[k] * c->mu[k] * c->mu[k]);
+        const double pc[5] = {1.0, kPhiC1, kPhiC2, kPhiC3, kPhiC4};
+        for (int j = 0; j < 5; ++j) g.pc[j][k] = (float)(pc[j] / std::pow(c->mu[k], j + 1));
         wmu_sum += c->w[k] * c->mu[k];
     }
     g.wmu_sum = (float)wmu_sum;

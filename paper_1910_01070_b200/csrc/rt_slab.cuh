@@ -1,12 +1,14 @@
 // rt_slab.cuh -- fused steps 1-4, large-batch variant.
 //
-// One CTA = NW compute warps + 1 producer warp, working on ONE 32-point wavenumber tile
-// for NW models (compute warp w = model w of the group, lane = wavenumber).
+// One CTA = NW compute warps + 1 producer warp, working on ONE 64-point wavenumber tile
+// for NW models: compute warp w = model w of the group, each lane owns TWO adjacent
+// wavenumbers and does all of its fp32 arithmetic as packed pairs (FFMA2/FMUL2/FADD2,
+// sm_100 fma.rn.f32x2), which halves the issue slots of an issue-bound kernel.
 //
 // Table staging.  The levels are a fixed log-p grid, so the pressure cell of
 // level l is the same for every model.  Levels are grouped into SEGMENTS of constant pressure
 // cell; a segment needs two PLANES of the table, plane(ip) = sigma[all s][all iT][ip][tile]
-// (S*nT rows of 128 B).  The producer thread streams the planes through a ring of NB shared
+// (S*nT rows of 256 B).  The producer thread streams the planes through a ring of NB shared
 // memory slots with TMA (cp.async.bulk.tensor.4d, one box per species, mbarrier completion);
 // consumers release a slot through an "empty" mbarrier when they leave the last segment that
 // needs it.  Every table row is therefore read from L2 once per CTA and reused by all NW
@@ -14,11 +16,14 @@
 //
 // Cell walk.  VMRs are constant with height, so with G_c = sum_s x_s sigma_s at
 // the four corners c of the model's current (T, p) cell, chi_l = n_l sum_c b_c G_c (b = bilinear
-// weights): the species sum is redone only when the model enters another cell (every ~5 levels),
-// not at every level.  Algebraically identical to interpolating each species and then summing
-// (PAPER.md:241, 127); only the fp32 summation order differs.
+// weights): the species sum is redone only for the corners that change when the model enters
+// another cell (every ~5 levels), not at every level.  Algebraically identical to interpolating
+// each species and then summing; only the fp32 summation order differs.
 //
-// RT, Planck, optical depth: as in rt_direct.cuh (Eq. 2, 4-9), state in registers.
+// RT (Eq. 4-9) in the scaled deviation form H_k = (I_k - S_l) / mu_k:
+//   large dtau/mu_k:  H <- e H + (1 - e) q,            e = 2^(-dtau log2e / mu_k), q = dS / dtau
+//   small dtau/mu_k:  H <- H + P_k(dtau) (dS - dtau H), P_k(dtau) = phi(dtau/mu_k) / mu_k
+// (common.cuh, R10); Planck and optical depth as in rt_direct.cuh.
 #pragma once
 #include <cuda.h>
 
@@ -26,7 +31,7 @@
 
 namespace helios {
 
-constexpr int kSlabTile = 32;       // wavenumbers per CTA (one 128 B row segment per table row)
+constexpr int kSlabTile = 64;       // wavenumbers per CTA (one 256 B row segment per table row)
 constexpr int kSlabMaxRing = 8;
 
 struct SlabArgs {
@@ -83,7 +88,30 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, ui
         ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
-// shared memory: [ring][S*nT*32] planes | [C*nT*32] CIA | [NW][x_floats] | mbarriers
+__device__ __forceinline__ float2 bc2(float v) { return make_float2(v, v); }
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+
+// ga = sum_s x_s qa[s], gb = sum_s x_s qb[s]  (rows of species s are `stride` float2 apart)
+__device__ __forceinline__ void mix_pair(const float2* qa, const float2* qb, const float* x, int n, int stride,
+                                         float2& ga, float2& gb) {
+    ga = make_float2(0.0f, 0.0f); gb = ga;
+#pragma unroll 2
+    for (int s = 0; s < n; ++s) {
+        const float2 xs = bc2(x[s]);
+        ga = __ffma2_rn(xs, *qa, ga);
+        gb = __ffma2_rn(xs, *qb, gb);
+        qa += stride; qb += stride;
+    }
+}
+__device__ __forceinline__ void mix_one(const float2* qa, const float* x, int n, int stride, float2& ga) {
+    ga = make_float2(0.0f, 0.0f);
+    for (int s = 0; s < n; ++s) {
+        ga = __ffma2_rn(bc2(x[s]), *qa, ga);
+        qa += stride;
+    }
+}
+
+// shared memory: [ring][S*nT*64] planes | [C*nT*64] CIA | [NW][x_floats] | mbarriers
 __host__ __device__ inline size_t slab_plane_floats(int S, int nT) { return (size_t)S * nT * kSlabTile; }
 __host__ __device__ inline size_t slab_fixed_bytes(int C, int nT, int NW, int x_floats) {
     return sizeof(float) * ((size_t)C * nT * kSlabTile + (size_t)NW * x_floats) + 8 * (2 * kSlabMaxRing + 1) + 128;
@@ -136,7 +164,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
         return;
     }
 
-    // ===== consumers: warp = model, lane = wavenumber =====
+    // ===== consumers: warp = model, lane = two adjacent wavenumbers =====
     int b = group * NW + warp;
     const bool model_valid = b < a.B;
     if (!model_valid) b = a.B - 1;           // still takes part in the slot hand-shake
@@ -144,73 +172,103 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     for (int i = lane; i < a.x_floats; i += 32) xw[i] = a.model_x[(size_t)b * a.x_floats + i];
     __syncwarp();
 
-    const int inu = tile * kSlabTile + lane;
-    const double nu_d = a.nu0 + a.dnu * (double)inu;
-    const float nu = (float)nu_d;
-    const float nu_lo = (float)(nu_d - (double)nu);
-    const float c1nu3 = (float)(kC1 * nu_d * nu_d * nu_d);
-    const int row = a.nT * kSlabTile;         // floats between species in a plane
-    const float4* rec4 = reinterpret_cast<const float4*>(a.rec + (size_t)b * a.L * kSlabRecFloats);
+    const int inu = tile * kSlabTile + 2 * lane;
+    const double nu_d0 = a.nu0 + a.dnu * (double)inu, nu_d1 = a.nu0 + a.dnu * (double)(inu + 1);
+    const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
+    const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
+    const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
+    constexpr int kRow2 = kSlabTile / 2;      // float2 per table row
+    const int sp2 = a.nT * kRow2;             // float2 between species in a plane
+    const float4* rp = reinterpret_cast<const float4*>(a.rec + (size_t)b * a.L * kSlabRecFloats);
+    const float2* planes2 = reinterpret_cast<const float2*>(planes) + lane;
+    const float2* cia2 = reinterpret_cast<const float2*>(cia_s) + lane;
+    const float* xc = xw + a.S;
 
-    float J[A];
+    float2 H[A];
 #pragma unroll
-    for (int k = 0; k < A; ++k) J[k] = 0.0f;
-    float chi_prev = 0.0f, S_prev = 0.0f, hdz_prev = 0.0f;
-    float G00 = 0.0f, G01 = 0.0f, G10 = 0.0f, G11 = 0.0f, Gc0 = 0.0f, Gc1 = 0.0f;
-    int released = 0;
+    for (int k = 0; k < A; ++k) H[k] = make_float2(0.0f, 0.0f);
+    float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
+    float hdz_prev = 0.0f;
+    float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
+    int released = 0, cur_iT = -2, prev_lo = -1;
 
     if (a.C > 0) mbar_wait(cia_bar, 0);
 
     for (int seg = 0; seg < a.n_seg; ++seg) {
         const int l_begin = a.seg_lbegin[seg], l_end = a.seg_lbegin[seg + 1];
-        const float* pLo = planes + lane;
-        const float* pHi = planes + lane;
+        const float2* pLo = planes2;
+        const float2* pHi = planes2;
+        bool shifted = false;                 // the previous segment's lower plane is this one's upper plane
         if (a.S > 0) {
             const int eHi = a.seg_hi[seg], eLo = a.seg_lo[seg];
             mbar_wait(&full[eHi % NB], (uint32_t)((eHi / NB) & 1));
             mbar_wait(&full[eLo % NB], (uint32_t)((eLo / NB) & 1));
-            pHi += (size_t)(eHi % NB) * plane_floats;
-            pLo += (size_t)(eLo % NB) * plane_floats;
+            pHi += (size_t)(eHi % NB) * (plane_floats / 2);
+            pLo += (size_t)(eLo % NB) * (plane_floats / 2);
+            shifted = eHi == prev_lo;
+            prev_lo = eLo;
         }
-        int cur_iT = -1;
-        for (int l = l_begin; l < l_end; ++l) {
-            const float4 r0 = __ldg(rec4 + 3 * l), r1 = __ldg(rec4 + 3 * l + 1), r2 = __ldg(rec4 + 3 * l + 2);
+        bool fresh = true;
+        for (int l = l_begin; l < l_end; ++l, rp += 3) {
+            const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2);
             const int iT = __float_as_int(r2.y);
-            if (iT != cur_iT) {               // warp-uniform: the model entered another table cell
+            if (fresh || iT != cur_iT) {      // warp-uniform: the model is in another table cell
+                const float2* lo = pLo + iT * kRow2;
+                const float2* hi = pHi + iT * kRow2;
+                const float2* qc = cia2 + iT * kRow2;
+                if (!fresh && iT == cur_iT - 1) {            // one cell colder: (iT+1) corners are the old iT corners
+                    G10 = G00; G11 = G01; Gc1 = Gc0;
+                    mix_pair(lo, hi, xw, a.S, sp2, G00, G01);
+                    mix_one(qc, xc, a.C, sp2, Gc0);
+                } else if (!fresh && iT == cur_iT + 1) {     // one cell hotter
+                    G00 = G10; G01 = G11; Gc0 = Gc1;
+                    mix_pair(lo + kRow2, hi + kRow2, xw, a.S, sp2, G10, G11);
+                    mix_one(qc + kRow2, xc, a.C, sp2, Gc1);
+                } else if (fresh && shifted && iT == cur_iT) {   // next pressure cell, same temperature cell
+                    G01 = G00; G11 = G10;
+                    mix_pair(lo, lo + kRow2, xw, a.S, sp2, G00, G10);
+                } else {
+                    mix_pair(lo, lo + kRow2, xw, a.S, sp2, G00, G10);
+                    mix_pair(hi, hi + kRow2, xw, a.S, sp2, G01, G11);
+                    mix_pair(qc, qc + kRow2, xc, a.C, sp2, Gc0, Gc1);
+                }
                 cur_iT = iT;
-                const float* qLo = pLo + iT * kSlabTile;
-                const float* qHi = pHi + iT * kSlabTile;
-                G00 = G01 = G10 = G11 = 0.0f;
-                for (int s = 0; s < a.S; ++s) {
-                    const float x = xw[s];
-                    G00 = fmaf(x, qLo[s * row], G00);
-                    G10 = fmaf(x, qLo[s * row + kSlabTile], G10);
-                    G01 = fmaf(x, qHi[s * row], G01);
-                    G11 = fmaf(x, qHi[s * row + kSlabTile], G11);
-                }
-                Gc0 = Gc1 = 0.0f;
-                const float* qc = cia_s + iT * kSlabTile + lane;
-                for (int c = 0; c < a.C; ++c) {
-                    const float x = xw[a.S + c];
-                    Gc0 = fmaf(x, qc[c * row], Gc0);
-                    Gc1 = fmaf(x, qc[c * row + kSlabTile], Gc1);
-                }
+                fresh = false;
             }
-            float chi = r0.x * G00;
-            chi = fmaf(r0.y, G01, chi);
-            chi = fmaf(r0.z, G10, chi);
-            chi = fmaf(r0.w, G11, chi);
-            chi = fmaf(r1.x, Gc0, chi);
-            chi = fmaf(r1.y, Gc1, chi);
-            const float E = planck_E(r1.z, r1.w, nu, nu_lo);
-            const float Sl = planck_from_E(c1nu3, E);
+            float2 chi = __fmul2_rn(bc2(r0.x), G00);
+            chi = __ffma2_rn(bc2(r0.y), G01, chi);
+            chi = __ffma2_rn(bc2(r0.z), G10, chi);
+            chi = __ffma2_rn(bc2(r0.w), G11, chi);
+            chi = __ffma2_rn(bc2(r1.x), Gc0, chi);
+            chi = __ffma2_rn(bc2(r1.y), Gc1, chi);
+            // S_l = B_nu(T_l) = c1 nu^3 E / (1 - E), E = 2^(-a nu), a nu carried as a two-float product
+            const float2 ah = bc2(r1.z);
+            const float2 pr = __fmul2_rn(ah, nu);
+            float2 rr = __ffma2_rn(ah, nu, neg2(pr));
+            rr = __ffma2_rn(bc2(r1.w), nu, rr);
+            rr = __ffma2_rn(ah, nu_lo, rr);
+            const float2 E0 = make_float2(ex2_approx(-pr.x), ex2_approx(-pr.y));
+            const float2 E = __ffma2_rn(__fmul2_rn(E0, bc2(-0.69314718056f)), rr, E0);
+            const float2 om = __fadd2_rn(bc2(1.0f), neg2(E));
+            const float2 Sl = __fmul2_rn(c1nu3, __fmul2_rn(E, make_float2(rcp_approx(om.x), rcp_approx(om.y))));
             if (l > 0) {
-                const float dtau = (chi + chi_prev) * hdz_prev;
-                const float dS = S_prev - Sl;
-                const float q = dS * rcp_approx(dtau);
+                const float2 dtau = __fmul2_rn(__fadd2_rn(chi, chi_prev), bc2(hdz_prev));
+                const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
+                const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
+                const float2 ndtau = neg2(dtau);
 #pragma unroll
-                for (int k = 0; k < A; ++k)
-                    sc_update(J[k], dtau, q, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
+                for (int k = 0; k < A; ++k) {
+                    const float2 arg = __fmul2_rn(ndtau, bc2(a.ang.c_exp[k]));
+                    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+                    const float2 big = __ffma2_rn(e, H[k], __ffma2_rn(neg2(e), q, q));
+                    float2 P = __ffma2_rn(dtau, bc2(a.ang.pc[4][k]), bc2(a.ang.pc[3][k]));
+                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[2][k]));
+                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[1][k]));
+                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[0][k]));
+                    const float2 small = __ffma2_rn(P, __ffma2_rn(ndtau, H[k], dS), H[k]);
+                    H[k].x = dtau.x < a.ang.thr[k] ? small.x : big.x;
+                    H[k].y = dtau.y < a.ang.thr[k] ? small.y : big.y;
+                }
             }
             chi_prev = chi; S_prev = Sl; hdz_prev = r2.x;
         }
@@ -226,12 +284,19 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 
     if (!model_valid || inu >= a.nNu) return;
     float* out = a.flux + (size_t)b * a.flux_stride + inu;
-    if (a.model_flag[b]) { *out = __int_as_float(0x7fc00000); return; }
-    // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = J_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
-    float acc = S_prev * a.ang.wmu_sum;
+    const bool two = inu + 1 < a.nNu;
+    if (a.model_flag[b]) {
+        out[0] = __int_as_float(0x7fc00000);
+        if (two) out[1] = __int_as_float(0x7fc00000);
+        return;
+    }
+    // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = mu_k H_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
+    float2 acc = __fmul2_rn(S_prev, bc2(a.ang.wmu_sum));
 #pragma unroll
-    for (int k = 0; k < A; ++k) acc = fmaf(a.ang.wmu[k], J[k], acc);
-    *out = a.model_scale[b] * acc;
+    for (int k = 0; k < A; ++k) acc = __ffma2_rn(bc2(a.ang.wH[k]), H[k], acc);
+    const float scale = a.model_scale[b];
+    out[0] = scale * acc.x;
+    if (two) out[1] = scale * acc.y;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -248,8 +313,8 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
     SlabPlan p;
     if (A < 1 || A > kMaxAngles || nT > 256) return p;
     const int nw = want_nw > 0 ? want_nw : 16;
-    if (nw != 8 && nw != 12 && nw != 16) return p;
-    const int target_ctas = nw == 8 ? 3 : 2;
+    if (nw != 8 && nw != 16 && nw != 24) return p;
+    const int target_ctas = nw == 8 ? 3 : 1;
     const size_t plane = sizeof(float) * slab_plane_floats(S, nT);
     const size_t fixed = slab_fixed_bytes(C, nT, nw, slab_x_floats(S, C));
     for (int ctas = target_ctas; ctas >= 1; --ctas) {
@@ -284,8 +349,8 @@ inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& t
                                     cudaStream_t stream) {
     switch (p.NW) {
         case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p.smem, stream);
-        case 12: return launch_rt_slab_t<A, 12, 2>(tms, tmc, a, p.smem, stream);
-        case 16: return launch_rt_slab_t<A, 16, 2>(tms, tmc, a, p.smem, stream);
+        case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p.smem, stream);
+        case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p.smem, stream);
         default: return cudaErrorInvalidValue;
     }
 }
