@@ -110,11 +110,15 @@ class ClockSampler:
         return out
 
 
-def oracle_sample_size(cfg, cores):
-    """Bounded sample: about 10-30 s of CPU work (measured ~0.8 core-s per model at configs[2])."""
-    per_model = 6e-9 * cfg.n_nu * cfg.n_levels * (4 * cfg.n_species + 2 * cfg.n_cia + 3 * cfg.n_angles + 6)
-    n = int(max(1, min(cfg.batch, round(20.0 / max(per_model, 1e-3)))))
-    return max(min(n, cfg.batch), min(cores, cfg.batch))
+def oracle_sample_size(wl, cfg, cores, target_s=15.0):
+    """Bounded sample: about `target_s` seconds of wall time on all cores.  One model per core is
+    timed first (a fraction of a second to a few seconds) and the count scaled from that."""
+    probe = min(cores, cfg.batch)
+    dt, _ = time_oracle(wl, probe)
+    per_model_core_s = dt * min(cores, probe) / probe
+    n = int(target_s * cores / max(per_model_core_s, 1e-4))
+    n = max(probe, (n // cores) * cores if n >= cores else n)
+    return max(1, min(n, cfg.batch))
 
 
 def time_oracle(wl, n_models, repeats=1):
@@ -138,8 +142,8 @@ def run_reference(args):
     wl = workloads.make_workload(args.config, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls)
     import oracle
     cores = oracle.max_threads()
-    n = oracle_sample_size(cfg, cores)
-    n = max(1, min(n, max(cores, n // max(1, args.steps // 2))))   # keep K+W steps within minutes
+    # keep the whole --steps K --warmup W run within a few minutes: ~60 s of oracle time in total
+    n = oracle_sample_size(wl, cfg, cores, target_s=min(15.0, 60.0 / max(1, args.steps)))
     for _ in range(args.warmup):
         time_oracle(wl, min(n, cores))
     t = [time_oracle(wl, n)[0] for _ in range(args.steps)]
@@ -288,7 +292,7 @@ def run_gpu(args):
     }
     if world == 1 and not args.no_cpu_baseline:
         import oracle
-        n = oracle_sample_size(cfg, oracle.max_threads())
+        n = oracle_sample_size(wl, cfg, oracle.max_threads())
         dt, cores = time_oracle(wl, n)
         line["cpu_baseline"] = {"value": n / dt, "unit": "models/s", "cores": cores, "kind": "oracle",
                                 "sample": f"first {n} of {cfg.batch} models of configs[{cfg.index}], "
