@@ -91,23 +91,35 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, ui
 __device__ __forceinline__ float2 bc2(float v) { return make_float2(v, v); }
 __device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
 
-// ga = sum_s x_s qa[s], gb = sum_s x_s qb[s]  (rows of species s are `stride` float2 apart)
-__device__ __forceinline__ void mix_pair(const float2* qa, const float2* qb, const float* x, int n, int stride,
+__device__ __forceinline__ float2 lds_f2(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds_f1(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+// ga = sum_s x_s row_a[s], gb = sum_s x_s row_b[s].  qa, qb, x: shared-memory byte addresses;
+// rows of consecutive species are `stride` bytes apart.
+__device__ __forceinline__ void mix_pair(uint32_t qa, uint32_t qb, uint32_t x, int n, uint32_t stride,
                                          float2& ga, float2& gb) {
     ga = make_float2(0.0f, 0.0f); gb = ga;
-#pragma unroll 2
+#pragma unroll 4
     for (int s = 0; s < n; ++s) {
-        const float2 xs = bc2(x[s]);
-        ga = __ffma2_rn(xs, *qa, ga);
-        gb = __ffma2_rn(xs, *qb, gb);
-        qa += stride; qb += stride;
+        const float2 xs = bc2(lds_f1(x));
+        ga = __ffma2_rn(xs, lds_f2(qa), ga);
+        gb = __ffma2_rn(xs, lds_f2(qb), gb);
+        qa += stride; qb += stride; x += 4;
     }
 }
-__device__ __forceinline__ void mix_one(const float2* qa, const float* x, int n, int stride, float2& ga) {
+__device__ __forceinline__ void mix_one(uint32_t qa, uint32_t x, int n, uint32_t stride, float2& ga) {
     ga = make_float2(0.0f, 0.0f);
+#pragma unroll 2
     for (int s = 0; s < n; ++s) {
-        ga = __ffma2_rn(bc2(x[s]), *qa, ga);
-        qa += stride;
+        ga = __ffma2_rn(bc2(lds_f1(x)), lds_f2(qa), ga);
+        qa += stride; x += 4;
     }
 }
 
@@ -177,12 +189,13 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
     const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
     const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
-    constexpr int kRow2 = kSlabTile / 2;      // float2 per table row
-    const int sp2 = a.nT * kRow2;             // float2 between species in a plane
+    constexpr uint32_t kRowB = kSlabTile * sizeof(float);   // bytes per table row in a plane
+    const uint32_t spB = a.nT * kRowB;        // bytes between species in a plane
     const float4* rp = reinterpret_cast<const float4*>(a.rec + (size_t)b * a.L * kSlabRecFloats);
-    const float2* planes2 = reinterpret_cast<const float2*>(planes) + lane;
-    const float2* cia2 = reinterpret_cast<const float2*>(cia_s) + lane;
-    const float* xc = xw + a.S;
+    const uint32_t planes_a = smem_u32(planes) + lane * 8;   // shared-memory byte addresses of this lane's pair
+    const uint32_t cia_a = smem_u32(cia_s) + lane * 8;
+    const uint32_t xw_a = smem_u32(xw), xc_a = xw_a + a.S * 4;
+    const uint32_t plane_bytes = (uint32_t)(plane_floats * sizeof(float));
 
     float2 H[A];
 #pragma unroll
@@ -196,15 +209,14 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 
     for (int seg = 0; seg < a.n_seg; ++seg) {
         const int l_begin = a.seg_lbegin[seg], l_end = a.seg_lbegin[seg + 1];
-        const float2* pLo = planes2;
-        const float2* pHi = planes2;
+        uint32_t pLo = planes_a, pHi = planes_a;
         bool shifted = false;                 // the previous segment's lower plane is this one's upper plane
         if (a.S > 0) {
             const int eHi = a.seg_hi[seg], eLo = a.seg_lo[seg];
             mbar_wait(&full[eHi % NB], (uint32_t)((eHi / NB) & 1));
             mbar_wait(&full[eLo % NB], (uint32_t)((eLo / NB) & 1));
-            pHi += (size_t)(eHi % NB) * (plane_floats / 2);
-            pLo += (size_t)(eLo % NB) * (plane_floats / 2);
+            pHi += (uint32_t)(eHi % NB) * plane_bytes;
+            pLo += (uint32_t)(eLo % NB) * plane_bytes;
             shifted = eHi == prev_lo;
             prev_lo = eLo;
         }
@@ -213,24 +225,22 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2);
             const int iT = __float_as_int(r2.y);
             if (fresh || iT != cur_iT) {      // warp-uniform: the model is in another table cell
-                const float2* lo = pLo + iT * kRow2;
-                const float2* hi = pHi + iT * kRow2;
-                const float2* qc = cia2 + iT * kRow2;
+                const uint32_t lo = pLo + iT * kRowB, hi = pHi + iT * kRowB, qc = cia_a + iT * kRowB;
                 if (!fresh && iT == cur_iT - 1) {            // one cell colder: (iT+1) corners are the old iT corners
                     G10 = G00; G11 = G01; Gc1 = Gc0;
-                    mix_pair(lo, hi, xw, a.S, sp2, G00, G01);
-                    mix_one(qc, xc, a.C, sp2, Gc0);
+                    mix_pair(lo, hi, xw_a, a.S, spB, G00, G01);
+                    mix_one(qc, xc_a, a.C, spB, Gc0);
                 } else if (!fresh && iT == cur_iT + 1) {     // one cell hotter
                     G00 = G10; G01 = G11; Gc0 = Gc1;
-                    mix_pair(lo + kRow2, hi + kRow2, xw, a.S, sp2, G10, G11);
-                    mix_one(qc + kRow2, xc, a.C, sp2, Gc1);
+                    mix_pair(lo + kRowB, hi + kRowB, xw_a, a.S, spB, G10, G11);
+                    mix_one(qc + kRowB, xc_a, a.C, spB, Gc1);
                 } else if (fresh && shifted && iT == cur_iT) {   // next pressure cell, same temperature cell
                     G01 = G00; G11 = G10;
-                    mix_pair(lo, lo + kRow2, xw, a.S, sp2, G00, G10);
+                    mix_pair(lo, lo + kRowB, xw_a, a.S, spB, G00, G10);
                 } else {
-                    mix_pair(lo, lo + kRow2, xw, a.S, sp2, G00, G10);
-                    mix_pair(hi, hi + kRow2, xw, a.S, sp2, G01, G11);
-                    mix_pair(qc, qc + kRow2, xc, a.C, sp2, Gc0, Gc1);
+                    mix_pair(lo, lo + kRowB, xw_a, a.S, spB, G00, G10);
+                    mix_pair(hi, hi + kRowB, xw_a, a.S, spB, G01, G11);
+                    mix_pair(qc, qc + kRowB, xc_a, a.C, spB, Gc0, Gc1);
                 }
                 cur_iT = iT;
                 fresh = false;
