@@ -491,7 +491,11 @@ static SlabPlan plan_slab(const helios_ctx* c, int B) {
     SlabPlan none;
     if (c->opt_kernel == 1 || !c->have_tmaps) return none;
     if (c->opt_kernel == 0 && B < 8) return none;      // a few models: the direct kernel streams the table once
-    return slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, c->opt_models_per_cta, c->smem_optin, c->smem_sm);
+    // models per CTA (measured on B200, configs 1-3): 24 warps hide latency best while the state fits
+    // 72 registers (<= 4 angles); 16 otherwise; 8 for batches too small to fill 16-model groups
+    int nw = c->opt_models_per_cta;
+    if (nw == 0) nw = B < 16 ? 8 : (c->A <= 4 && B >= 128 ? 24 : 16);
+    return slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, nw, c->smem_optin, c->smem_sm);
 }
 
 int helios_reserve(helios_ctx* c, int B) {
