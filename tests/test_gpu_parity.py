@@ -40,6 +40,11 @@ def wl2(torch_cuda):
     return W.make_workload(2, device=_gen_device(torch_cuda))
 
 
+@pytest.fixture(scope="module")
+def wl3(torch_cuda):
+    return W.make_workload(3, device=_gen_device(torch_cuda))
+
+
 def _run(torch, wl, params, kernel=0, highres=True, models_per_cta=0):
     from paper_1910_01070_b200 import Helios
     h = Helios(0)
@@ -107,6 +112,55 @@ def test_config2_full_batch_sampled_models(torch_cuda, oracle, wl2):
     assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
     # properties that hold for every model at any size
     assert np.isfinite(spec).all() and np.isfinite(logl).all() and (flux > 0).all()
+
+
+def test_config3_full_batch_sampled_models(torch_cuda, oracle, wl3):
+    """configs[3] at its full size (B = 1024, 85001 wavenumbers, 150 levels, 8 angles, 1.6 GB of
+    tables) in the launch configuration bench.py times; the oracle recomputes a seeded sample."""
+    spec, logl, flux, st = _run(torch_cuda, wl3, wl3.params, kernel=0)
+    rng = np.random.default_rng(3)
+    pick = np.sort(rng.choice(wl3.cfg.batch, 6, replace=False))
+    ref = oracle.forward_workload(wl3, params=wl3.params[pick], want_flux=True)
+    assert _relerr(flux[pick], ref["flux_hr"]) <= TOL_FLUX
+    assert _relerr(spec[pick], ref["spectra"]) <= TOL_FLUX
+    assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
+    assert np.isfinite(spec).all() and np.isfinite(logl).all() and (flux > 0).all()
+
+
+def test_config4_streamed_loglike_only(torch_cuda, oracle, wl3):
+    """configs[4]: 4096 parameter vectors as 16 back-to-back helios_loglike_batch calls of 256 on
+    one stream, no host synchronisation in between, spectra never written.  logL must equal what
+    helios_forward_batch returns for the same vectors, and the oracle's on a seeded sample."""
+    from paper_1910_01070_b200 import Helios
+    torch = torch_cuda
+    cfg4 = W.get_config(4)
+    params = W.draw_params(cfg4)
+    assert params.shape[0] == 4096
+    h = Helios(0)
+    h.setup_workload(wl3)                       # config 4 re-uses config 3's tables, grid and observation
+    h.set_kernel(2)                             # same kernel for the 256-model calls and the 4-model check
+    p = torch.as_tensor(params, device="cuda:0")
+    out = torch.empty(4096, dtype=torch.float64, device="cuda:0")
+    B = 4096 // cfg4.n_calls
+    for c in range(cfg4.n_calls):
+        h.loglike_batch(p[c * B:(c + 1) * B], out[c * B:(c + 1) * B])
+    pick = np.sort(np.random.default_rng(4).choice(4096, 4, replace=False))
+    _, full = h.forward_batch(p[torch.as_tensor(pick, device="cuda:0")].contiguous())
+    torch.cuda.synchronize()
+    logl = out.cpu().numpy()
+    assert np.isfinite(logl).all()
+    assert np.array_equal(full.cpu().numpy(), logl[pick])
+    ref = oracle.forward_workload(wl3, params=params[pick])
+    assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
+    h.close()
+
+
+def test_logl_near_truth_config3(torch_cuda, oracle, wl3):
+    params = W.near_truth_params(wl3.cfg, 4)
+    ref = oracle.forward_workload(wl3, params=params)
+    spec, logl, _, _ = _run(torch_cuda, wl3, params, 0, highres=False)
+    assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
+    assert np.max(np.abs(logl - ref["logl"])) <= TOL_LOGL_ABS
 
 
 @pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
