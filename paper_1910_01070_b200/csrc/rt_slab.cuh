@@ -90,6 +90,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, ui
 
 __device__ __forceinline__ float2 bc2(float v) { return make_float2(v, v); }
 __device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+// A register copy the compiler may not rename away: keeps the corner values in FIXED registers
+// across the level loop, so the (rare) cell changes pay for the moves and the steady state has none.
+__device__ __forceinline__ void hard_copy(float2& dst, const float2& src) {
+    asm volatile("mov.b32 %0, %2;\n\tmov.b32 %1, %3;" : "=f"(dst.x), "=f"(dst.y) : "f"(src.x), "f"(src.y));
+}
 
 __device__ __forceinline__ float2 lds_f2(uint32_t addr) {
     float2 v;
@@ -227,15 +232,15 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             if (fresh || iT != cur_iT) {      // warp-uniform: the model is in another table cell
                 const uint32_t lo = pLo + iT * kRowB, hi = pHi + iT * kRowB, qc = cia_a + iT * kRowB;
                 if (!fresh && iT == cur_iT - 1) {            // one cell colder: (iT+1) corners are the old iT corners
-                    G10 = G00; G11 = G01; Gc1 = Gc0;
+                    hard_copy(G10, G00); hard_copy(G11, G01); hard_copy(Gc1, Gc0);
                     mix_pair(lo, hi, xw_a, a.S, spB, G00, G01);
                     mix_one(qc, xc_a, a.C, spB, Gc0);
                 } else if (!fresh && iT == cur_iT + 1) {     // one cell hotter
-                    G00 = G10; G01 = G11; Gc0 = Gc1;
+                    hard_copy(G00, G10); hard_copy(G01, G11); hard_copy(Gc0, Gc1);
                     mix_pair(lo + kRowB, hi + kRowB, xw_a, a.S, spB, G10, G11);
                     mix_one(qc + kRowB, xc_a, a.C, spB, Gc1);
                 } else if (fresh && shifted && iT == cur_iT) {   // next pressure cell, same temperature cell
-                    G01 = G00; G11 = G10;
+                    hard_copy(G01, G00); hard_copy(G11, G10);
                     mix_pair(lo, lo + kRowB, xw_a, a.S, spB, G00, G10);
                 } else {
                     mix_pair(lo, lo + kRowB, xw_a, a.S, spB, G00, G10);
