@@ -63,6 +63,32 @@ struct AngleSet {
 constexpr double kPhiC1 = -0.49999951482099264, kPhiC2 = 0.16665108206599635, kPhiC3 = -0.041490654102785796,
                  kPhiC4 = 0.00751360621792363;
 
+// Gauss-Legendre rule of order n = 1..8 on [-1,1] mapped to mu in (0,1): mu = (x+1)/2, w = W/2
+// (R12).  Compile-time copy for the staged kernel, whose per-angle
+// constants are instruction immediates; helios_set_atmosphere() checks it against the Newton
+// solution it computes at run time.
+constexpr double kGLmu[8][8] = {
+    {0.5, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0},
+    {0.21132486540518713, 0.7886751345948129, 1.0, 1.0, 1.0, 1.0, 1.0, 1.0},
+    {0.1127016653792583, 0.5, 0.8872983346207417, 1.0, 1.0, 1.0, 1.0, 1.0},
+    {0.06943184420297371, 0.33000947820757187, 0.6699905217924281, 0.9305681557970262, 1.0, 1.0, 1.0, 1.0},
+    {0.04691007703066802, 0.23076534494715845, 0.5, 0.7692346550528415, 0.9530899229693319, 1.0, 1.0, 1.0},
+    {0.03376524289842403, 0.16939530676686776, 0.38069040695840156, 0.6193095930415985, 0.8306046932331322, 0.9662347571015759, 1.0, 1.0},
+    {0.0254460438286207, 0.12923440720030277, 0.2970774243113014, 0.5, 0.7029225756886985, 0.8707655927996972, 0.9745539561713793, 1.0},
+    {0.019855071751231912, 0.10166676129318664, 0.2372337950418355, 0.4082826787521751, 0.5917173212478248, 0.7627662049581645, 0.8983332387068134, 0.9801449282487681},
+};
+constexpr double kGLw[8][8] = {
+    {1.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0},
+    {0.5, 0.5, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0},
+    {0.27777777777777785, 0.4444444444444444, 0.27777777777777785, 0.0, 0.0, 0.0, 0.0, 0.0},
+    {0.17392742256872679, 0.3260725774312732, 0.3260725774312732, 0.17392742256872679, 0.0, 0.0, 0.0, 0.0},
+    {0.11846344252809464, 0.23931433524968315, 0.28444444444444433, 0.23931433524968315, 0.11846344252809464, 0.0, 0.0, 0.0},
+    {0.08566224618958514, 0.18038078652406936, 0.23395696728634552, 0.23395696728634552, 0.18038078652406936, 0.08566224618958514, 0.0, 0.0},
+    {0.06474248308443487, 0.13985269574463843, 0.19091502525255935, 0.20897959183673465, 0.19091502525255935, 0.13985269574463843, 0.06474248308443487, 0.0},
+    {0.05061426814518853, 0.11119051722668721, 0.15685332293894344, 0.18134189168918083, 0.18134189168918083, 0.15685332293894344, 0.11119051722668721, 0.05061426814518853},
+};
+__host__ __device__ constexpr double cpow(double b, int e) { double r = 1.0; for (int i = 0; i < e; ++i) r *= b; return r; }
+
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));

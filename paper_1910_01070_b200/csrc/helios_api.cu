@@ -397,6 +397,10 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
         wmu_sum += c->w[k] * c->mu[k];
     }
     g.wmu_sum = (float)wmu_sum;
+    // the staged kernel uses the compile-time copy of this rule (common.cuh): they must agree
+    for (int k = 0; k < A; ++k)
+        if (std::fabs(c->mu[k] - kGLmu[A - 1][k]) > 1e-14 || std::fabs(c->w[k] - kGLw[A - 1][k]) > 1e-14)
+            return fail(c, HELIOS_ECUDA, "internal: Gauss-Legendre table mismatch at n = %d, k = %d", A, k);
     c->have_atmo = true;
     c->cap_B = 0;
     return HELIOS_OK;

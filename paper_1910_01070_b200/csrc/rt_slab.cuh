@@ -27,12 +27,15 @@
 #pragma once
 #include <cuda.h>
 
+#include <utility>
+
 #include "common.cuh"
 
 namespace helios {
 
 constexpr int kSlabTile = 64;       // wavenumbers per CTA (one 256 B row segment per table row)
 constexpr int kSlabMaxRing = 8;
+constexpr uint32_t kMbarSuspendNs = 20000;   // try_wait suspend-time hint: sleep in hardware instead of polling
 
 struct SlabArgs {
     int S, C, nT, nNu, L, B;
@@ -70,11 +73,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "{\n\t"
         ".reg .pred p;\n\t"
         "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
         "@p bra DONE_%=;\n\t"
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+        "}" ::"r"(smem_u32(bar)), "r"(parity), "r"(kMbarSuspendNs) : "memory");
 }
 // TMA: one box of the 4-D table view {nu, ip, iT, s} / the 3-D CIA view {nu, iT, c} -> shared memory
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
@@ -126,6 +129,42 @@ __device__ __forceinline__ void mix_one(uint32_t qa, uint32_t x, int n, uint32_t
         ga = __ffma2_rn(bc2(lds_f1(x)), lds_f2(qa), ga);
         qa += stride; x += 4;
     }
+}
+
+// One angle of one layer for a pair of wavenumbers (state H = (I - S_l)/mu_k).  All per-angle
+// constants are compile-time (Gauss-Legendre order A, node K) and become instruction immediates.
+template <int A, int K>
+__device__ __forceinline__ void angle_step(float2& H, float2 dtau, float2 ndtau, float2 q, float2 dS) {
+    constexpr double mu = kGLmu[A - 1][K];
+    constexpr float c_exp = (float)(kLog2e / mu), thr = (float)(0.25 * mu);
+    constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                    p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+    const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+    const float2 big = __ffma2_rn(e, H, __ffma2_rn(neg2(e), q, q));
+    float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+    P = __ffma2_rn(dtau, P, bc2(p2));
+    P = __ffma2_rn(dtau, P, bc2(p1));
+    P = __ffma2_rn(dtau, P, bc2(p0));
+    const float2 small = __ffma2_rn(P, __ffma2_rn(ndtau, H, dS), H);
+    H.x = dtau.x < thr ? small.x : big.x;
+    H.y = dtau.y < thr ? small.y : big.y;
+}
+template <int A, int... K>
+__device__ __forceinline__ void all_angles(float2 (&H)[A], float2 dtau, float2 ndtau, float2 q, float2 dS,
+                                           std::integer_sequence<int, K...>) {
+    (angle_step<A, K>(H[K], dtau, ndtau, q, dS), ...);
+}
+template <int A, int K>
+__device__ __forceinline__ void flux_term(float2& acc, float2 H) {
+    constexpr float wH = (float)(kGLw[A - 1][K] * kGLmu[A - 1][K] * kGLmu[A - 1][K]);
+    acc = __ffma2_rn(bc2(wH), H, acc);
+}
+template <int A, int... K>
+__device__ __forceinline__ float2 flux_sum(const float2 (&H)[A], float2 S_top, std::integer_sequence<int, K...>) {
+    float2 acc = __fmul2_rn(S_top, bc2(0.5f));    // sum_k w_k mu_k = 1/2: the rule integrates mu exactly
+    (flux_term<A, K>(acc, H[K]), ...);
+    return acc;
 }
 
 // shared memory: [ring][S*nT*64] planes | [C*nT*64] CIA | [NW][x_floats] | mbarriers
@@ -271,19 +310,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
                 const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
                 const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
                 const float2 ndtau = neg2(dtau);
-#pragma unroll
-                for (int k = 0; k < A; ++k) {
-                    const float2 arg = __fmul2_rn(ndtau, bc2(a.ang.c_exp[k]));
-                    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
-                    const float2 big = __ffma2_rn(e, H[k], __ffma2_rn(neg2(e), q, q));
-                    float2 P = __ffma2_rn(dtau, bc2(a.ang.pc[4][k]), bc2(a.ang.pc[3][k]));
-                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[2][k]));
-                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[1][k]));
-                    P = __ffma2_rn(dtau, P, bc2(a.ang.pc[0][k]));
-                    const float2 small = __ffma2_rn(P, __ffma2_rn(ndtau, H[k], dS), H[k]);
-                    H[k].x = dtau.x < a.ang.thr[k] ? small.x : big.x;
-                    H[k].y = dtau.y < a.ang.thr[k] ? small.y : big.y;
-                }
+                all_angles<A>(H, dtau, ndtau, q, dS, std::make_integer_sequence<int, A>{});
             }
             chi_prev = chi; S_prev = Sl; hdz_prev = r2.x;
         }
@@ -306,9 +333,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
         return;
     }
     // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = mu_k H_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
-    float2 acc = __fmul2_rn(S_prev, bc2(a.ang.wmu_sum));
-#pragma unroll
-    for (int k = 0; k < A; ++k) acc = __ffma2_rn(bc2(a.ang.wH[k]), H[k], acc);
+    const float2 acc = flux_sum<A>(H, S_prev, std::make_integer_sequence<int, A>{});
     const float scale = a.model_scale[b];
     out[0] = scale * acc.x;
     if (two) out[1] = scale * acc.y;
