@@ -65,6 +65,7 @@ struct helios_ctx {
     float* d_rec = nullptr; size_t rec_bytes = 0;
     float* d_flux = nullptr; long long flux_stride = 0;
     float* d_scale = nullptr; int* d_flag = nullptr; float* d_model_x = nullptr;
+    double* d_obs_partial = nullptr; unsigned* d_obs_arrived = nullptr;
     unsigned long long* d_counters = nullptr;    // [2]
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
@@ -118,6 +119,7 @@ static void free_all(helios_ctx* c) {
     dfree(c->d_seg_lbegin); dfree(c->d_seg_hi); dfree(c->d_seg_lo); dfree(c->d_load_ip);
     dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x); dfree(c->d_counters);
+    dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
 }
 
@@ -510,6 +512,7 @@ int helios_reserve(helios_ctx* c, int B) {
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x);
+    dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
     c->cap_B = 0;
     const int rf = std::max(direct_rec_floats(c->S, c->C), kSlabRecFloats);
@@ -519,6 +522,12 @@ int helios_reserve(helios_ctx* c, int B) {
     CU_TRY(c, cudaMalloc(&c->d_scale, sizeof(float) * B));
     CU_TRY(c, cudaMalloc(&c->d_flag, sizeof(int) * B));
     CU_TRY(c, cudaMalloc(&c->d_model_x, sizeof(float) * (size_t)B * slab_x_floats(c->S, c->C)));
+    {
+        const int n_chunks = ((c->J > 0 ? c->J : 1) + kObsBinsPerCta - 1) / kObsBinsPerCta;
+        CU_TRY(c, cudaMalloc(&c->d_obs_partial, sizeof(double) * (size_t)B * n_chunks));
+        CU_TRY(c, cudaMalloc(&c->d_obs_arrived, sizeof(unsigned) * B));
+        CU_TRY(c, cudaMemsetAsync(c->d_obs_arrived, 0, sizeof(unsigned) * B, c->stream));
+    }
     CU_TRY(c, cudaMalloc(&c->d_params_stage, sizeof(double) * (size_t)B * (2 + c->K + c->S)));
     CU_TRY(c, cudaMalloc(&c->d_spectra_stage, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
     CU_TRY(c, cudaMalloc(&c->d_logl_stage, sizeof(double) * B));
@@ -624,7 +633,8 @@ int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spec
     oa.J = c->J; oa.row_ptr = c->d_row_ptr; oa.row_lo = c->d_row_lo; oa.W = c->d_W; oa.flux = c->d_flux;
     oa.flux_stride = c->flux_stride; oa.model_flag = c->d_flag; oa.obs = c->d_obs; oa.inv2var = c->d_inv2var;
     oa.logl_const = c->logl_const; oa.spectra = spectra_out; oa.logl = logl_out;
-    k_obs_apply<<<B, kObsThreads, 0, c->stream>>>(oa);
+    oa.partial = c->d_obs_partial; oa.arrived = c->d_obs_arrived;
+    k_obs_apply<<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
     stamp(c, 3);

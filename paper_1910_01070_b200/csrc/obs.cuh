@@ -85,21 +85,30 @@ struct ObsApplyArgs {
     double logl_const;        // -1/2 sum_j ln(2 pi sigma_j^2)
     float* spectra;           // DEVICE [B][J] or nullptr
     double* logl;             // DEVICE [B] or nullptr
+    double* partial;          // DEVICE [B][n_chunks] chi-square of each bin chunk (workspace)
+    unsigned* arrived;        // DEVICE [B] chunks finished per model; zero between launches (workspace)
 };
 
 constexpr int kObsThreads = 256;
+constexpr int kObsBinsPerCta = 64;   // 8 warps x 8 bins
 
-// One CTA per model.  Each warp owns bins j = warp, warp + 8, ...: lanes stride the band,
-// a shuffle tree finishes M_j, lane 0 adds the chi-square term in fp64.  The per-warp
-// partial sums are combined in a fixed order, so logL is bitwise reproducible.
+// One CTA per (model, chunk of 64 bins): B * J / 64 CTAs keep every SM busy (one CTA per model
+// left 14 warps per SM waiting on dependent L2 loads).  Each warp owns 8 bins: lanes stride the
+// band of W, a shuffle tree finishes M_j, lane 0 adds the chi-square term in fp64.  The chunk
+// sums go to `partial`; the CTA that finishes a model last (atomic ticket) adds them in chunk
+// order, so logL is bitwise reproducible, and only logL is written when spectra == nullptr.
 __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
     __shared__ double warp_sum[kObsThreads / 32];
-    const int b = blockIdx.x;
+    __shared__ unsigned ticket;
+    const int b = blockIdx.y, chunk = blockIdx.x, n_chunks = gridDim.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int kPerWarp = kObsBinsPerCta / (kObsThreads / 32);
     const bool bad = a.model_flag[b] != 0;
     const float* F = a.flux + (size_t)b * a.flux_stride;
     double chi2 = 0.0;
-    for (int j = warp; j < a.J; j += kObsThreads / 32) {
+    const int j0 = chunk * kObsBinsPerCta + warp * kPerWarp;
+#pragma unroll 2
+    for (int j = j0; j < min(j0 + kPerWarp, a.J); ++j) {
         const int p0 = a.row_ptr[j], len = a.row_ptr[j + 1] - p0;
         const float* w = a.W + p0;
         const float* f = F + a.row_lo[j];
@@ -122,13 +131,21 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
             }
         }
     }
-    if (a.logl) {
-        if (lane == 0) warp_sum[warp] = chi2;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double s = 0.0;
-            for (int w = 0; w < kObsThreads / 32; ++w) s += warp_sum[w];
-            a.logl[b] = bad ? -CUDART_INF : a.logl_const - s;
+    if (!a.logl) return;
+    if (lane == 0) warp_sum[warp] = chi2;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < kObsThreads / 32; ++w) s += warp_sum[w];
+        a.partial[(size_t)b * n_chunks + chunk] = s;
+        __threadfence();
+        ticket = atomicAdd(&a.arrived[b], 1u);
+        if (ticket == (unsigned)n_chunks - 1) {          // every chunk of this model is in `partial`
+            __threadfence();
+            double t = 0.0;
+            for (int c = 0; c < n_chunks; ++c) t += __ldcg(&a.partial[(size_t)b * n_chunks + c]);
+            a.logl[b] = bad ? -CUDART_INF : a.logl_const - t;
+            a.arrived[b] = 0;
         }
     }
 }
