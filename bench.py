@@ -180,6 +180,9 @@ def run_gpu(args):
     dev = torch.device("cuda", local)
 
     cfg = workloads.get_config(args.config)
+    if args.batch > 0:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, batch=args.batch * cfg.n_calls)
     n_calls = cfg.n_calls                       # configs[4]: 16 back-to-back calls per step
     B_call = cfg.batch // n_calls
     wl = workloads.make_workload(args.config, batch=cfg.batch, device="cuda")
@@ -312,6 +315,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 slab")
     ap.add_argument("--models-per-cta", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="override the workload's batch size (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -496,7 +496,6 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
 static SlabPlan plan_slab(const helios_ctx* c, int B) {
     SlabPlan none;
     if (c->opt_kernel == 1 || !c->have_tmaps) return none;
-    if (c->opt_kernel == 0 && B < 8) return none;      // a few models: the direct kernel streams the table once
     // models per CTA (measured on B200, configs 1-3): 24 warps hide latency best while the state fits
     // 72 registers (<= 4 angles); 16 otherwise; 8 for batches too small to fill 16-model groups
     int nw = c->opt_models_per_cta;
