@@ -10,4 +10,6 @@ from .binding import (  # noqa: F401
     interp_sigma, interp_cia, number_density, chi_level, layer_thickness, layer_dtau,
     planck, gauss_legendre_01, sc_coefficients, flux_one_nu, convolve, bin_spectrum,
     loglike, forward, max_threads, forward_workload,
+    loglike_inflated, lobatto_nodes, tp_dofs_from_ratios, temperature_profile_fe, teff, cloud_dtau,
+    EXTRA_DISTANCE, EXTRA_ERROR_INFLATION, EXTRA_GREY_CLOUD,
 )

@@ -83,6 +83,25 @@ def lib():
             C.c_int, _dp, _dp, _dp, _dp,
             C.c_int, _dp, _dp, _dp, _dp, C.c_int]
         L.oracle_forward.restype = C.c_long
+        L.oracle_forward_ext.argtypes = [
+            C.c_int, C.c_int, _dp, C.c_int, _dp, C.c_int, C.c_double, C.c_double, _fp,
+            C.c_int, _fp,
+            C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+            C.c_int, _dp, _dp, _dp, _dp,
+            C.c_int, _dp, _dp, _dp, _dp, C.c_int, C.c_int, C.c_int, C.c_int, C.c_uint, C.c_double, C.c_double, _dp]
+        L.oracle_forward_ext.restype = C.c_long
+        L.oracle_loglike_inflated.argtypes = [C.c_int, _dp, _dp, _dp, C.c_double]
+        L.oracle_loglike_inflated.restype = C.c_double
+        L.oracle_lobatto_nodes.argtypes = [C.c_int, _dp]
+        L.oracle_lobatto_nodes.restype = C.c_int
+        L.oracle_tp_dofs_from_ratios.argtypes = [C.c_int, _dp, _dp]
+        L.oracle_tp_dofs_from_ratios.restype = None
+        L.oracle_temperature_profile_fe.argtypes = [C.c_int, _dp, C.c_int, C.c_int, _dp, C.c_double, C.c_double, _dp]
+        L.oracle_temperature_profile_fe.restype = C.c_int
+        L.oracle_teff.argtypes = [C.c_int, C.c_double, C.c_double, _dp, C.c_double, C.c_double]
+        L.oracle_teff.restype = C.c_double
+        L.oracle_cloud_dtau.argtypes = [C.c_int, _dp, C.c_double, C.c_double, C.c_double, _dp]
+        L.oracle_cloud_dtau.restype = None
         L.oracle_max_threads.argtypes = []
         L.oracle_max_threads.restype = C.c_int
         _lib = L
@@ -241,11 +260,61 @@ def loglike(D, err, M):
     return float(lib().oracle_loglike(len(d), dpp, ep, mp))
 
 
+EXTRA_DISTANCE, EXTRA_ERROR_INFLATION, EXTRA_GREY_CLOUD = 1, 2, 4
+
+
+def loglike_inflated(D, err, M, eps):
+    d, dpp = _d(D)
+    e, ep = _d(err)
+    m, mp = _d(M)
+    return float(lib().oracle_loglike_inflated(len(d), dpp, ep, mp, float(eps)))
+
+
+def lobatto_nodes(q):
+    out = np.empty(q + 1, np.float64)
+    if lib().oracle_lobatto_nodes(int(q), out.ctypes.data_as(_dp)):
+        raise ValueError("order must be 1..4")
+    return out
+
+
+def tp_dofs_from_ratios(theta):
+    t, tp = _d(theta)
+    out = np.empty(len(t), np.float64)
+    lib().oracle_tp_dofs_from_ratios(len(t), tp, out.ctypes.data_as(_dp))
+    return out
+
+
+def temperature_profile_fe(p_bar, n_elements, order, T_dof, p_bottom_bar, p_top_bar):
+    p, pp = _d(p_bar)
+    t, tp = _d(T_dof)
+    assert len(t) == n_elements * order + 1
+    out = np.empty(len(p), np.float64)
+    if lib().oracle_temperature_profile_fe(len(p), pp, int(n_elements), int(order), tp, float(p_bottom_bar),
+                                           float(p_top_bar), out.ctypes.data_as(_dp)):
+        raise ValueError("bad element count / order")
+    return out
+
+
+def teff(nu0, dnu, F_plus, nu_a, nu_b):
+    f, fp = _d(F_plus)
+    return float(lib().oracle_teff(len(f), float(nu0), float(dnu), fp, float(nu_a), float(nu_b)))
+
+
+def cloud_dtau(p_bar, tau_c, p_top_c, phi):
+    p, pp = _d(p_bar)
+    out = np.zeros(max(len(p) - 1, 1), np.float64)
+    lib().oracle_cloud_dtau(len(p), pp, float(tau_c), float(p_top_c), float(phi), out.ctypes.data_as(_dp))
+    return out[:len(p) - 1]
+
+
 def forward(T_grid, log10p_grid, nu0, dnu, sigma, cia, n_levels, p_bottom_bar, p_top_bar,
             n_knots, n_angles, mean_mol_weight, he_to_h2, flux_const,
             bin_edges, obs, obs_err, inst_sigma, params,
-            want_flux=False, want_spectra=True, want_logl=True, n_threads=0):
-    """Whole path.  Returns dict(flux_hr, spectra, logl, n_clamped)."""
+            want_flux=False, want_spectra=True, want_logl=True, n_threads=0,
+            tp_elements=0, tp_order=1, tp_ratio=False, extras=0, teff_range=None):
+    """Whole path.  Returns dict(flux_hr, spectra, logl, n_clamped[, teff]).
+    tp_elements/tp_order/tp_ratio, extras (EXTRA_* flags) and teff_range = (nu_a, nu_b)
+    switch on the NEXT rows (oracle_forward_ext)."""
     sg, sgp = _f(sigma)
     S, nT, nP, nNu = sg.shape
     if cia is None or len(cia) == 0:
@@ -258,7 +327,10 @@ def forward(T_grid, log10p_grid, nu0, dnu, sigma, cia, n_levels, p_bottom_bar, p
     ed, edp = _d(bin_edges)
     J = len(ed) - 1
     par, parp = _d(params)
-    par = par.reshape(-1, 2 + n_knots + S)
+    n_t = tp_elements * tp_order + 1 if tp_elements > 0 else n_knots
+    n_extra = (1 if extras & EXTRA_DISTANCE else 0) + (1 if extras & EXTRA_ERROR_INFLATION else 0) + \
+              (3 if extras & EXTRA_GREY_CLOUD else 0)
+    par = par.reshape(-1, 2 + n_t + S + n_extra)
     B = par.shape[0]
     if want_logl:
         ob, obp = _d(obs)
@@ -272,19 +344,24 @@ def forward(T_grid, log10p_grid, nu0, dnu, sigma, cia, n_levels, p_bottom_bar, p
     flux = np.empty((B, nNu), np.float64) if want_flux else None
     spec = np.empty((B, J), np.float64) if want_spectra else None
     logl = np.empty(B, np.float64) if want_logl else None
-    ncl = lib().oracle_forward(
+    teff = np.empty(B, np.float64) if teff_range is not None else None
+    ncl = lib().oracle_forward_ext(
         S, nT, tgp, nP, pgp, nNu, float(nu0), float(dnu), sgp, Cn, cp,
         int(n_levels), float(p_bottom_bar), float(p_top_bar), int(n_knots), int(n_angles),
         float(mean_mol_weight), float(he_to_h2), float(flux_const),
         J, edp, obp, erp, isp, B, parp,
         flux.ctypes.data_as(_dp) if want_flux else None,
         spec.ctypes.data_as(_dp) if want_spectra else None,
-        logl.ctypes.data_as(_dp) if want_logl else None, int(n_threads))
-    return dict(flux_hr=flux, spectra=spec, logl=logl, n_clamped=int(ncl))
+        logl.ctypes.data_as(_dp) if want_logl else None, int(n_threads),
+        int(tp_elements), int(tp_order), int(bool(tp_ratio)), int(extras),
+        float(teff_range[0]) if teff_range is not None else 0.0,
+        float(teff_range[1]) if teff_range is not None else 0.0,
+        teff.ctypes.data_as(_dp) if teff is not None else None)
+    return dict(flux_hr=flux, spectra=spec, logl=logl, n_clamped=int(ncl), teff=teff)
 
 
 def forward_workload(wl, params=None, want_flux=False, want_spectra=True, want_logl=True,
-                     n_threads=0, obs=None, obs_err=None):
+                     n_threads=0, obs=None, obs_err=None, **ext):
     """Convenience: run the oracle on a workloads.Workload."""
     cfg = wl.cfg
     obs = wl.obs if obs is None else obs
@@ -297,4 +374,4 @@ def forward_workload(wl, params=None, want_flux=False, want_spectra=True, want_l
                    wl.bin_edges, obs, obs_err, wl.inst_sigma,
                    wl.params if params is None else params,
                    want_flux=want_flux, want_spectra=want_spectra, want_logl=want_logl,
-                   n_threads=n_threads)
+                   n_threads=n_threads, **ext)

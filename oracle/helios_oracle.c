@@ -362,6 +362,108 @@ double oracle_loglike(int J, const double *D, const double *err, const double *M
     return lnL;
 }
 
+/* ========================================================================
+ * Rows NEXT-1 .. NEXT-4 of SURVEY.md 8(f)
+ * ====================================================================== */
+
+/* NEXT-1.  Eq. 22-23: s_j^2 = sigma_j^2 + 10^eps,
+ *   ln L = sum_j ( -(D_j - M_j)^2/(2 s_j^2) - 1/2 ln(2 pi s_j^2) )
+ * (R20: the second term belongs inside the sum, as in Eq. 19). */
+double oracle_loglike_inflated(int J, const double *D, const double *err, const double *M, double eps)
+{
+    double lnL = 0.0, add = pow(10.0, eps);
+    for (int j = 0; j < J; ++j) {
+        double s2 = err[j] * err[j] + add;                      /* Eq. 22 */
+        double r = D[j] - M[j];
+        lnL += -(r * r) / (2.0 * s2) - 0.5 * log(2.0 * PI * s2);  /* Eq. 23 */
+    }
+    return lnL;
+}
+
+/* NEXT-2.  Sect. 2.5.1.  Gauss-Lobatto points of the
+ * reference element [0,1] for order q = 1..4 (N_p = q + 1, Eq. 14): the end
+ * points plus the roots of P'_q mapped from [-1,1]. */
+int oracle_lobatto_nodes(int q, double *xi)
+{
+    switch (q) {
+        case 1: xi[0] = 0.0; xi[1] = 1.0; return 0;
+        case 2: xi[0] = 0.0; xi[1] = 0.5; xi[2] = 1.0; return 0;
+        case 3: { double a = 1.0 / sqrt(5.0);
+                  xi[0] = 0.0; xi[1] = 0.5 * (1.0 - a); xi[2] = 0.5 * (1.0 + a); xi[3] = 1.0; return 0; }
+        case 4: { double a = sqrt(3.0 / 7.0);
+                  xi[0] = 0.0; xi[1] = 0.5 * (1.0 - a); xi[2] = 0.5; xi[3] = 0.5 * (1.0 + a); xi[4] = 1.0; return 0; }
+        default: return -1;
+    }
+}
+
+/* "The only, actually retrieved temperature is the one at the bottom ...  For all
+ * other temperatures, we retrieve a parameter b, such that, e.g., T_2 = b_2 T_1"
+ * (PAPER.md:219); b is "the slope between two adjacent temperature nodes", so each
+ * ratio refers to the node below it (R28): T_i = b_i T_{i-1}.  theta = (T_1, b_2..b_N). */
+void oracle_tp_dofs_from_ratios(int N, const double *theta, double *T_dof)
+{
+    T_dof[0] = theta[0];
+    for (int i = 1; i < N; ++i) T_dof[i] = theta[i] * T_dof[i - 1];
+}
+
+/* Eq. 12-15: K_e elements equidistant in log p from p_bot (element 0) to p_top,
+ * order q, continuous: element k owns the global dofs k q .. k q + q (N_T = K_e q + 1,
+ * Eq. 16); inside an element T is the Lagrange interpolant (Eq. 13) through the
+ * Gauss-Lobatto points of the reference element. */
+int oracle_temperature_profile_fe(int L, const double *p_bar, int Ke, int q, const double *T_dof,
+                                  double p_bot_bar, double p_top_bar, double *T)
+{
+    double xi_n[8];
+    if (Ke < 1 || oracle_lobatto_nodes(q, xi_n)) return -1;
+    double x_bot = log10(p_bot_bar), x_top = log10(p_top_bar);
+    for (int l = 0; l < L; ++l) {
+        double s = (log10(p_bar[l]) - x_bot) / (x_top - x_bot) * (double)Ke;
+        int k = (int)floor(s);
+        if (k < 0) k = 0;
+        if (k > Ke - 1) k = Ke - 1;
+        double xi = s - (double)k;                       /* reference element coordinate */
+        double Tl = 0.0;
+        for (int i = 0; i <= q; ++i) {
+            double ell = 1.0;                            /* Eq. 13 */
+            for (int j = 0; j <= q; ++j) if (j != i) ell *= (xi - xi_n[j]) / (xi_n[i] - xi_n[j]);
+            Tl += T_dof[k * q + i] * ell;                /* Eq. 12 */
+        }
+        T[l] = Tl;
+    }
+    return 0;
+}
+
+/* NEXT-3.  Sect. 2.6: the outgoing flux F+ integrated over
+ * [nu_a, nu_b] (the paper: 1-20 micron) "converted into an effective temperature by
+ * using the Stefan-Boltzmann law".  Quadrature (R30): trapezoid on the grid with
+ * linearly interpolated end points, i.e. the bin rule O6 times the width. */
+void oracle_bin(int nNu, double nu0, double dnu, const double *Fd, int J, const double *edges, double *M);
+double oracle_teff(int nNu, double nu0, double dnu, const double *Fplus, double nu_a, double nu_b)
+{
+    const double sigma_sb = 2.0 * pow(PI, 5) * pow(K_BOLTZMANN, 4) /
+                            (15.0 * pow(H_PLANCK, 3) * C_LIGHT * C_LIGHT);
+    double e[2] = {nu_a, nu_b}, mean;
+    oracle_bin(nNu, nu0, dnu, Fplus, 1, e, &mean);
+    return pow(mean * (nu_b - nu_a) / sigma_sb, 0.25);
+}
+
+/* NEXT-4.  App. B: a grey cloud with "three free parameters: the
+ * cloud optical depth, the pressure of the cloud layer top, and the bottom of the cloud
+ * layer, defined as the fraction of the top pressure".  Reading R29: p_bot = p_top (1 + phi);
+ * the vertical optical depth tau_c is spread uniformly in pressure over [p_top, p_bot]; layer l
+ * (levels l, l+1) receives the share of its pressure overlap; the part of the cloud outside the
+ * modelled range is dropped.  dtau_cloud[l], l = 0 .. L-2, is added to dtau_l at every nu. */
+void oracle_cloud_dtau(int L, const double *p_bar, double tau_c, double p_top_c, double phi, double *dtau_cloud)
+{
+    double p_bot_c = p_top_c * (1.0 + phi);
+    for (int l = 0; l + 1 < L; ++l) {
+        double hi = p_bar[l] < p_bot_c ? p_bar[l] : p_bot_c;            /* larger pressure end */
+        double lo = p_bar[l + 1] > p_top_c ? p_bar[l + 1] : p_top_c;
+        double overlap = hi - lo;
+        dtau_cloud[l] = overlap > 0.0 ? tau_c * overlap / (p_bot_c - p_top_c) : 0.0;
+    }
+}
+
 /* ------------------------------------------------------------------------
  * Whole path for B parameter vectors (OpenMP over models only).
  * params [B][P], P = 2 + K + S: log10 g (cgs), f, T_knot[0..K-1] (bottom->top),
@@ -371,7 +473,17 @@ double oracle_loglike(int J, const double *D, const double *err, const double *M
  * gets NaN spectra and logl = -inf (R-nonfinite).
  * Returns the number of (model, level) pairs whose (T, p) was clamped.
  * ---------------------------------------------------------------------- */
-long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *log10p_grid,
+#define ORACLE_EXTRA_DISTANCE        1u   /* + d:   F = F+ f flux_const / d^2 (Eq. 9, flux_const = R_*^2)   */
+#define ORACLE_EXTRA_ERROR_INFLATION 2u   /* + eps: Eq. 22-23                                                */
+#define ORACLE_EXTRA_GREY_CLOUD      4u   /* + log10 tau_c, log10 p_top [bar], log10 phi (App. B, R29)        */
+
+/* Extended driver.  Temperature parameters: tp_elements = 0 -> K nodal temperatures, linear in
+ * log p (the hot path); tp_elements = K_e > 0 -> K_e elements of order tp_order (N_T = K_e q + 1
+ * values), nodal temperatures (tp_ratio = 0) or (T_1, b_2 .. b_N) (tp_ratio = 1).
+ * params [B][P], P = 2 + N_T + S + extras: log10 g, f, temperature parameters, log10 VMR,
+ * then the extras that are switched on, in the order of the flags above.
+ * teff (or NULL): T_eff from F+ over [teff_nu_a, teff_nu_b] (NEXT-3). */
+long oracle_forward_ext(int S, int nT, const double *T_grid, int nP, const double *log10p_grid,
                     int nNu, double nu0, double dnu,
                     const float *sigma,            /* [S][nT][nP][nNu] */
                     int C, const float *cia,       /* [C][nT][nNu]     */
@@ -380,9 +492,15 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
                     int J, const double *edges, const double *obs, const double *err,
                     const double *inst_sigma,      /* [nNu] or NULL    */
                     int B, const double *params,
-                    double *flux_hr, double *spectra, double *logl, int n_threads)
+                    double *flux_hr, double *spectra, double *logl, int n_threads,
+                    int tp_elements, int tp_order, int tp_ratio, unsigned extras,
+                    double teff_nu_a, double teff_nu_b, double *teff)
 {
-    int P = 2 + K + S;
+    int NT = tp_elements > 0 ? tp_elements * tp_order + 1 : K;
+    int i_d = -1, i_eps = -1, i_cloud = -1, P = 2 + NT + S;
+    if (extras & ORACLE_EXTRA_DISTANCE) i_d = P++;
+    if (extras & ORACLE_EXTRA_ERROR_INFLATION) i_eps = P++;
+    if (extras & ORACLE_EXTRA_GREY_CLOUD) { i_cloud = P; P += 3; }
     long n_clamped = 0;
     double *mu = (double *)malloc(sizeof(double) * A), *w = (double *)malloc(sizeof(double) * A);
     oracle_gauss_legendre_01(A, mu, w);
@@ -398,19 +516,29 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
             if (flux_hr) for (int k = 0; k < nNu; ++k) flux_hr[(size_t)b * nNu + k] = NAN;
             if (spectra) for (int j = 0; j < J; ++j) spectra[(size_t)b * J + j] = NAN;
             if (logl) logl[b] = -INFINITY;
+            if (teff) teff[b] = NAN;
             continue;
         }
         double g_cgs = pow(10.0, th[0]);
         double f = th[1];
-        const double *T_knot = th + 2;
-        const double *log10_vmr = th + 2 + K;
+        const double *T_par = th + 2;
+        const double *log10_vmr = th + 2 + NT;
+        double scale = f * flux_const;                                              /* Eq. 9 */
+        if (i_d >= 0) scale /= th[i_d] * th[i_d];
 
         double *p_bar = (double *)malloc(sizeof(double) * L);
         double *T = (double *)malloc(sizeof(double) * L);
         double *x = (double *)malloc(sizeof(double) * (S > 0 ? S : 1));
         double x_h2, x_he;
         oracle_level_pressures(L, p_bot_bar, p_top_bar, p_bar);                     /* O0 */
-        oracle_temperature_profile(L, p_bar, K, T_knot, p_bot_bar, p_top_bar, T);   /* O0 */
+        if (tp_elements > 0) {                                                       /* NEXT-2 */
+            double *dof = (double *)malloc(sizeof(double) * NT);
+            if (tp_ratio) oracle_tp_dofs_from_ratios(NT, T_par, dof);
+            else for (int i = 0; i < NT; ++i) dof[i] = T_par[i];
+            oracle_temperature_profile_fe(L, p_bar, tp_elements, tp_order, dof, p_bot_bar, p_top_bar, T);
+            free(dof);
+        } else
+            oracle_temperature_profile(L, p_bar, K, T_par, p_bot_bar, p_top_bar, T);   /* O0 */
         oracle_mixing_ratios(S, log10_vmr, he_to_h2, x, &x_h2, &x_he);              /* O0 */
 
         /* chi[l][nu], then dtau[l][nu] */
@@ -446,6 +574,15 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
                               dtau + (size_t)l * nNu);
         }
 
+        if (i_cloud >= 0) {                                                          /* NEXT-4 */
+            double *dc = (double *)malloc(sizeof(double) * (L > 1 ? L - 1 : 1));
+            oracle_cloud_dtau(L, p_bar, pow(10.0, th[i_cloud]), pow(10.0, th[i_cloud + 1]),
+                              pow(10.0, th[i_cloud + 2]), dc);
+            for (int l = 0; l + 1 < L; ++l)
+                for (int k = 0; k < nNu; ++k) dtau[(size_t)l * nNu + k] += dc[l];
+            free(dc);
+        }
+
         /* O4: RT per wavenumber, then Eq. 9 */
         double *F = (double *)malloc(sizeof(double) * nNu);
         double *Scol = (double *)malloc(sizeof(double) * L);
@@ -455,8 +592,10 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
             for (int l = 0; l < L; ++l) Scol[l] = oracle_planck(nu, T[l]);
             for (int l = 0; l + 1 < L; ++l) dcol[l] = dtau[(size_t)l * nNu + k];
             double Fplus = oracle_flux_one_nu(L, Scol, dcol, A, mu, w);
-            F[k] = Fplus * f * flux_const;                                           /* Eq. 9 */
+            F[k] = Fplus;
         }
+        if (teff) teff[b] = oracle_teff(nNu, nu0, dnu, F, teff_nu_a, teff_nu_b);      /* NEXT-3 */
+        for (int k = 0; k < nNu; ++k) F[k] *= scale;                                 /* Eq. 9 */
         if (flux_hr) for (int k = 0; k < nNu; ++k) flux_hr[(size_t)b * nNu + k] = F[k];
 
         if (spectra || logl) {
@@ -465,7 +604,8 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
             oracle_convolve(nNu, nu0, dnu, F, inst_sigma, Fd);                       /* O5 */
             oracle_bin(nNu, nu0, dnu, Fd, J, edges, M);                              /* O6 */
             if (spectra) for (int j = 0; j < J; ++j) spectra[(size_t)b * J + j] = M[j];
-            if (logl) logl[b] = oracle_loglike(J, obs, err, M);                      /* O7 */
+            if (logl) logl[b] = i_eps >= 0 ? oracle_loglike_inflated(J, obs, err, M, th[i_eps])  /* NEXT-1 */
+                                           : oracle_loglike(J, obs, err, M);                      /* O7 */
             free(Fd); free(M);
         }
         for (int s = 0; s < S; ++s) free(sig[s]);
@@ -475,6 +615,20 @@ long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *l
     }
     free(mu); free(w);
     return n_clamped;
+}
+
+/* The hot path as BASELINE.json states it: K nodal temperatures, no extras. */
+long oracle_forward(int S, int nT, const double *T_grid, int nP, const double *log10p_grid,
+                    int nNu, double nu0, double dnu, const float *sigma, int C, const float *cia,
+                    int L, double p_bot_bar, double p_top_bar, int K, int A,
+                    double mmw, double he_to_h2, double flux_const,
+                    int J, const double *edges, const double *obs, const double *err,
+                    const double *inst_sigma, int B, const double *params,
+                    double *flux_hr, double *spectra, double *logl, int n_threads)
+{
+    return oracle_forward_ext(S, nT, T_grid, nP, log10p_grid, nNu, nu0, dnu, sigma, C, cia, L, p_bot_bar,
+                              p_top_bar, K, A, mmw, he_to_h2, flux_const, J, edges, obs, err, inst_sigma,
+                              B, params, flux_hr, spectra, logl, n_threads, 0, 1, 0, 0u, 0.0, 0.0, NULL);
 }
 
 int oracle_max_threads(void)
