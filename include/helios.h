@@ -94,6 +94,28 @@ int helios_set_atmosphere(helios_ctx* ctx, int n_levels, double p_bottom_bar, do
                           int n_knots, int n_angles, double mean_mol_weight, double he_to_h2,
                           double flux_const);
 
+/* Temperature parametrisation by finite elements (Sect. 2.5.1, Eq. 12-16):
+ * n_elements elements equidistant in log p between p_bottom and p_top, polynomial order 1..4,
+ * Gauss-Lobatto points on the reference element, continuous across elements, so the profile has
+ * N_T = n_elements * order + 1 temperature parameters (bottom -> top) which replace the n_knots
+ * values of helios_set_atmosphere in the parameter vector.
+ *   ratio_form = 0: the N_T nodal temperatures [K];
+ *   ratio_form = 1: T_1 and the ratios b_2 .. b_N with T_i = b_i T_{i-1} (R28).
+ * Call after helios_set_atmosphere (which selects n_knots nodes / first order again). */
+int helios_set_tp_elements(helios_ctx* ctx, int n_elements, int order, int ratio_form);
+
+/* Extra parameters appended to every parameter vector, in this order:
+ *   HELIOS_EXTRA_DISTANCE         d        Eq. 9 with flux_const = R_*^2: F = F+ f flux_const / d^2
+ *   HELIOS_EXTRA_ERROR_INFLATION  epsilon  Eq. 22-23: s_j^2 = sigma_j^2 + 10^epsilon in ln L
+ *   HELIOS_EXTRA_GREY_CLOUD       log10 tau_c, log10 p_top [bar], log10 phi   (App. B, R29: grey cloud
+ *                                 of vertical optical depth tau_c between p_top and p_top (1 + phi)) */
+#define HELIOS_EXTRA_DISTANCE        1u
+#define HELIOS_EXTRA_ERROR_INFLATION 2u
+#define HELIOS_EXTRA_GREY_CLOUD      4u
+int helios_set_extras(helios_ctx* ctx, unsigned flags);
+/* HOST out: P = 2 + N_T + n_species + number of extras, the row length of `params`. */
+int helios_get_n_params(const helios_ctx* ctx, int* n_params_out);
+
 /* Observation (Eq. 17, 255, 267-270 Eq. 19).
  *   bin_edges_cm1 HOST [n_bins+1] ascending, inside [nu_0, nu_{nNu-1}]
  *   obs, obs_err  HOST [n_bins] (may both be NULL: spectra only, logL unavailable)
@@ -121,6 +143,13 @@ int helios_loglike_batch(helios_ctx* ctx, int B, const double* params, double* l
 /* Test hook: the flux of Eq. 9 on the native grid, before the instrument
  * profile.  flux_out: DEVICE [B][nNu] fp32.  Needs no observation. */
 int helios_forward_highres(helios_ctx* ctx, int B, const double* params, float* flux_out);
+
+/* Effective temperature (Sect. 2.6): the outgoing flux F+ of Eq. 8 (without the
+ * f (R/d)^2 of Eq. 9) integrated over [nu_a, nu_b] on the native grid (trapezoid, interpolated end
+ * points) and converted with the Stefan-Boltzmann law.  teff_out: DEVICE [B] fp64, Kelvin.
+ * Runs steps 0-4 of the hot path and one reduction kernel; needs no observation.  Enqueues only. */
+int helios_teff_batch(helios_ctx* ctx, int B, const double* params, double nu_a_cm1, double nu_b_cm1,
+                      double* teff_out);
 
 /* End-to-end variant: params, spectra_out (or NULL), logl_out (or NULL) are HOST
  * buffers (pinned for full speed).  Copies params to the device, runs the hot

@@ -22,6 +22,7 @@ HELIOS_OPT_KERNEL = 1
 HELIOS_OPT_MODELS_PER_CTA = 2
 HELIOS_OPT_TIMING = 3
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB = 0, 1, 2
+HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD = 1, 2, 4
 
 _dp = C.POINTER(C.c_double)
 _fp = C.POINTER(C.c_float)
@@ -71,11 +72,16 @@ def lib() -> C.CDLL:
         L.helios_get_stats.argtypes = [_vp, C.POINTER(helios_stats), C.c_int]
         L.helios_get_angles.argtypes = [_vp, _dp, _dp]
         L.helios_get_stage_ms.argtypes = [_vp, _dp, C.POINTER(C.c_int)]
+        L.helios_set_tp_elements.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
+        L.helios_set_extras.argtypes = [_vp, C.c_uint]
+        L.helios_get_n_params.argtypes = [_vp, C.POINTER(C.c_int)]
+        L.helios_teff_batch.argtypes = [_vp, C.c_int, _vp, C.c_double, C.c_double, _vp]
         for name in ("helios_create", "helios_set_stream", "helios_set_option", "helios_load_opacity",
                      "helios_set_atmosphere", "helios_set_observation", "helios_reserve",
                      "helios_forward_batch", "helios_loglike_batch", "helios_forward_highres",
                      "helios_forward_batch_host", "helios_get_stats", "helios_get_angles",
-                     "helios_get_stage_ms"):
+                     "helios_get_stage_ms", "helios_set_tp_elements", "helios_set_extras", "helios_get_n_params",
+                     "helios_teff_batch"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -161,6 +167,26 @@ def helios_set_observation(ctx: int, bin_edges, obs=None, obs_err=None, inst_sig
     if inst_sigma is not None:
         s, sp = _f64(inst_sigma)
     _check(ctx, lib().helios_set_observation(_vp(ctx), len(e) - 1, ep, op, rp, sp))
+
+
+def helios_set_tp_elements(ctx: int, n_elements: int, order: int, ratio_form: bool = False) -> None:
+    _check(ctx, lib().helios_set_tp_elements(_vp(ctx), int(n_elements), int(order), int(bool(ratio_form))))
+
+
+def helios_set_extras(ctx: int, flags: int) -> None:
+    _check(ctx, lib().helios_set_extras(_vp(ctx), int(flags)))
+
+
+def helios_get_n_params(ctx: int) -> int:
+    n = C.c_int()
+    _check(ctx, lib().helios_get_n_params(_vp(ctx), C.byref(n)))
+    return n.value
+
+
+def helios_teff_batch(ctx: int, params, nu_a_cm1: float, nu_b_cm1: float, teff_out) -> None:
+    """params: CUDA float64 [B][P]; teff_out: CUDA float64 [B]."""
+    _check(ctx, lib().helios_teff_batch(_vp(ctx), params.shape[0], _dev_ptr(params, "float64"), float(nu_a_cm1),
+                                        float(nu_b_cm1), _dev_ptr(teff_out, "float64")))
 
 
 def helios_reserve(ctx: int, max_batch: int) -> None:
@@ -313,6 +339,20 @@ class Helios:
 
     def forward_batch_host(self, params_host, spectra_out_host=None, logl_out_host=None):
         helios_forward_batch_host(self.ctx, params_host, spectra_out_host, logl_out_host)
+
+    def set_tp_elements(self, n_elements, order, ratio_form=False):
+        helios_set_tp_elements(self.ctx, n_elements, order, ratio_form)
+        self.n_params = helios_get_n_params(self.ctx)
+
+    def set_extras(self, flags):
+        helios_set_extras(self.ctx, flags)
+        self.n_params = helios_get_n_params(self.ctx)
+
+    def teff_batch(self, params, nu_a_cm1, nu_b_cm1):
+        import torch
+        out = torch.empty((params.shape[0],), dtype=torch.float64, device=params.device)
+        helios_teff_batch(self.ctx, params, nu_a_cm1, nu_b_cm1, out)
+        return out
 
     def set_timing(self, on: bool):
         helios_set_option(self.ctx, HELIOS_OPT_TIMING, 1 if on else 0)

@@ -42,7 +42,11 @@ struct helios_ctx {
     double p_bot = 0, p_top = 0, mmw = 0, he_to_h2 = 0, flux_const = 1;
     std::vector<double> mu, w;
     AngleSet ang{};
-    double* d_lvl_p = nullptr; int* d_lvl_knot = nullptr; double* d_lvl_xi = nullptr;
+    double* d_lvl_p = nullptr; int* d_lvl_elem = nullptr; double* d_lvl_lw = nullptr;
+    std::vector<double> lvl_p;          // level pressures, bar
+    int tp_order = 1, tp_ratio = 0, NT = 0;   // temperature parametrisation (helios_set_tp_elements)
+    unsigned extras = 0;                // HELIOS_EXTRA_* flags
+    int n_extra = 0;
     int* d_lvl_ip = nullptr; double* d_lvl_u = nullptr; int* d_lvl_pclamp = nullptr;
     double* d_lvl_lnratio = nullptr;
     std::vector<int> lvl_ip;
@@ -57,7 +61,8 @@ struct helios_ctx {
     bool have_obs = false, have_data = false;
     int J = 0;
     double logl_const = 0;
-    double* d_edges = nullptr; double* d_obs = nullptr; double* d_inv2var = nullptr;
+    double* d_edges = nullptr; double* d_obs = nullptr; double* d_inv2var = nullptr; double* d_var = nullptr;
+    double* d_addvar = nullptr;         // [cap_B] 10^epsilon per model
     int* d_row_ptr = nullptr; int* d_row_lo = nullptr; float* d_W = nullptr;
 
     // ---- workspace (grown on demand)
@@ -114,13 +119,44 @@ static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
 
 static void free_all(helios_ctx* c) {
     dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid);
-    dfree(c->d_lvl_p); dfree(c->d_lvl_knot); dfree(c->d_lvl_xi); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
+    dfree(c->d_lvl_p); dfree(c->d_lvl_elem); dfree(c->d_lvl_lw); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
     dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
     dfree(c->d_seg_lbegin); dfree(c->d_seg_hi); dfree(c->d_seg_lo); dfree(c->d_load_ip);
-    dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
+    dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_var); dfree(c->d_addvar); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x); dfree(c->d_counters);
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
+}
+
+static int n_params(const helios_ctx* c) { return 2 + c->NT + c->S + c->n_extra; }
+
+// Levels -> finite elements (Sect. 2.5.1): n_elements elements equidistant in log p, order q with
+// Gauss-Lobatto points on the reference element; per level the element index and the values of
+// the element's q + 1 Lagrange polynomials (Eq. 13).  q = 0: one isothermal value.
+static cudaError_t build_tp(helios_ctx* c, int n_elements, int q) {
+    std::vector<int> elem(c->L, 0);
+    std::vector<double> lw((size_t)c->L * kMaxTpNodes, 0.0);
+    double node[kMaxTpNodes] = {0.0, 1.0, 0.0, 0.0, 0.0};
+    if (q == 2) { node[1] = 0.5; node[2] = 1.0; }
+    if (q == 3) { const double a = 1.0 / std::sqrt(5.0); node[1] = 0.5 * (1.0 - a); node[2] = 0.5 * (1.0 + a); node[3] = 1.0; }
+    if (q == 4) { const double a = std::sqrt(3.0 / 7.0); node[1] = 0.5 * (1.0 - a); node[2] = 0.5; node[3] = 0.5 * (1.0 + a); node[4] = 1.0; }
+    const double x_bot = std::log10(c->p_bot), x_top = std::log10(c->p_top);
+    for (int l = 0; l < c->L; ++l) {
+        if (q == 0) { lw[(size_t)l * kMaxTpNodes] = 1.0; continue; }
+        const double s = (std::log10(c->lvl_p[l]) - x_bot) / (x_top - x_bot) * n_elements;
+        int k = (int)std::floor(s);
+        k = k < 0 ? 0 : (k > n_elements - 1 ? n_elements - 1 : k);
+        const double xi = s - k;
+        elem[l] = k;
+        for (int i = 0; i <= q; ++i) {
+            double ell = 1.0;
+            for (int j = 0; j <= q; ++j) if (j != i) ell *= (xi - node[j]) / (node[i] - node[j]);
+            lw[(size_t)l * kMaxTpNodes + i] = ell;
+        }
+    }
+    cudaError_t e = upload(c->d_lvl_elem, elem, c->stream);
+    if (e == cudaSuccess) e = upload(c->d_lvl_lw, lw, c->stream);
+    return e;
 }
 
 // TMA views of the resident tables for the staged kernel (cuTensorMapEncodeTiled, resolved through
@@ -329,24 +365,19 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
     c->L = L; c->K = K; c->A = A; c->p_bot = p_bot; c->p_top = p_top; c->mmw = mmw; c->he_to_h2 = he_to_h2;
     c->flux_const = flux_const;
 
-    std::vector<double> p(L), xi(L), u(L), lnr(L, 0.0);
-    std::vector<int> knot(L), ip(L), pcl(L);
-    const double x_bot = std::log10(p_bot), x_top = std::log10(p_top);
+    std::vector<double> p(L), u(L), lnr(L, 0.0);
+    std::vector<int> ip(L), pcl(L);
     for (int l = 0; l < L; ++l) {
         p[l] = p_bot * std::pow(p_top / p_bot, (double)l / (double)(L - 1));   // equidistant in log p
-        const double x = std::log10(p[l]);
-        double s = (K > 1) ? (x - x_bot) / (x_top - x_bot) * (K - 1) : 0.0;
-        int k = (int)std::floor(s);
-        if (k < 0) k = 0;
-        if (k > K - 2) k = K - 2 < 0 ? 0 : K - 2;
-        knot[l] = k; xi[l] = s - k;
-        axis_cell(c->lp_grid, x, ip[l], u[l], pcl[l]);
+        axis_cell(c->lp_grid, std::log10(p[l]), ip[l], u[l], pcl[l]);
     }
+    c->lvl_p = p;
+    // K nodal temperatures, linear in log p = K - 1 first-order elements (one value: isothermal)
+    c->tp_order = K > 1 ? 1 : 0; c->tp_ratio = 0; c->NT = K;
+    CU_TRY(c, build_tp(c, K > 1 ? K - 1 : 1, c->tp_order));
     for (int l = 0; l + 1 < L; ++l) lnr[l] = std::log(p[l] / p[l + 1]);
     c->lvl_ip = ip;
     CU_TRY(c, upload(c->d_lvl_p, p, c->stream));
-    CU_TRY(c, upload(c->d_lvl_knot, knot, c->stream));
-    CU_TRY(c, upload(c->d_lvl_xi, xi, c->stream));
     CU_TRY(c, upload(c->d_lvl_ip, ip, c->stream));
     CU_TRY(c, upload(c->d_lvl_u, u, c->stream));
     CU_TRY(c, upload(c->d_lvl_pclamp, pcl, c->stream));
@@ -486,6 +517,9 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
         c->logl_const = cst;
         CU_TRY(c, upload(c->d_obs, o, c->stream));
         CU_TRY(c, upload(c->d_inv2var, i2v, c->stream));
+        std::vector<double> var(J);
+        for (int j = 0; j < J; ++j) var[j] = err[j] * err[j];
+        CU_TRY(c, upload(c->d_var, var, c->stream));
         c->have_data = true;
     }
     c->have_obs = true;
@@ -512,7 +546,7 @@ int helios_reserve(helios_ctx* c, int B) {
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x);
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
-    dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
+    dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage); dfree(c->d_addvar);
     c->cap_B = 0;
     const int rf = std::max(direct_rec_floats(c->S, c->C), kSlabRecFloats);
     c->flux_stride = c->stride;
@@ -527,7 +561,8 @@ int helios_reserve(helios_ctx* c, int B) {
         CU_TRY(c, cudaMalloc(&c->d_obs_arrived, sizeof(unsigned) * B));
         CU_TRY(c, cudaMemsetAsync(c->d_obs_arrived, 0, sizeof(unsigned) * B, c->stream));
     }
-    CU_TRY(c, cudaMalloc(&c->d_params_stage, sizeof(double) * (size_t)B * (2 + c->K + c->S)));
+    CU_TRY(c, cudaMalloc(&c->d_params_stage, sizeof(double) * (size_t)B * n_params(c)));
+    CU_TRY(c, cudaMalloc(&c->d_addvar, sizeof(double) * B));
     CU_TRY(c, cudaMalloc(&c->d_spectra_stage, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
     CU_TRY(c, cudaMalloc(&c->d_logl_stage, sizeof(double) * B));
     c->cap_B = B;
@@ -539,16 +574,17 @@ static inline void stamp(helios_ctx* c, int which) {
 }
 
 // steps 0-4: params -> flux (DEVICE [B][flux_stride])
-static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride) {
+static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride, int unit_scale = 0) {
     const SlabPlan plan = plan_slab(c, B);
     if (c->opt_kernel == 2 && !plan.ok)
         return fail(c, HELIOS_EINVAL, "staged kernel requested but unavailable for this table shape (shared memory / TMA)");
     const int slab = plan.ok ? 1 : 0;
     const int rf = slab ? kSlabRecFloats : direct_rec_floats(c->S, c->C);
     PrepArgs pa{};
-    pa.params = params; pa.B = B; pa.P = 2 + c->K + c->S; pa.K = c->K; pa.S = c->S; pa.C = c->C; pa.L = c->L;
-    pa.nT = c->nT; pa.nP = c->nP; pa.T_grid = c->d_Tgrid; pa.lvl_p_bar = c->d_lvl_p; pa.lvl_knot = c->d_lvl_knot;
-    pa.lvl_xi = c->d_lvl_xi; pa.lvl_ip = c->d_lvl_ip; pa.lvl_u = c->d_lvl_u; pa.lvl_pclamp = c->d_lvl_pclamp;
+    pa.params = params; pa.B = B; pa.P = n_params(c); pa.K = c->K; pa.S = c->S; pa.C = c->C; pa.L = c->L;
+    pa.nT = c->nT; pa.nP = c->nP; pa.T_grid = c->d_Tgrid; pa.lvl_p_bar = c->d_lvl_p; pa.lvl_elem = c->d_lvl_elem;
+    pa.lvl_lw = c->d_lvl_lw; pa.tp_order = c->tp_order; pa.tp_ratio = c->tp_ratio; pa.NT = c->NT; pa.extras = c->extras;
+    pa.unit_scale = unit_scale; pa.model_addvar = c->d_addvar; pa.lvl_ip = c->d_lvl_ip; pa.lvl_u = c->d_lvl_u; pa.lvl_pclamp = c->d_lvl_pclamp;
     pa.lvl_lnratio = c->d_lvl_lnratio; pa.mmw = c->mmw; pa.he_to_h2 = c->he_to_h2; pa.flux_const = c->flux_const;
     pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
     pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
@@ -631,6 +667,7 @@ int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spec
     ObsApplyArgs oa{};
     oa.J = c->J; oa.row_ptr = c->d_row_ptr; oa.row_lo = c->d_row_lo; oa.W = c->d_W; oa.flux = c->d_flux;
     oa.flux_stride = c->flux_stride; oa.model_flag = c->d_flag; oa.obs = c->d_obs; oa.inv2var = c->d_inv2var;
+    if (c->extras & HELIOS_EXTRA_ERROR_INFLATION) { oa.var = c->d_var; oa.addvar = c->d_addvar; }
     oa.logl_const = c->logl_const; oa.spectra = spectra_out; oa.logl = logl_out;
     oa.partial = c->d_obs_partial; oa.arrived = c->d_obs_arrived;
     k_obs_apply<<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa);
@@ -646,13 +683,63 @@ int helios_loglike_batch(helios_ctx* c, int B, const double* params, double* log
     return helios_forward_batch(c, B, params, nullptr, logl_out);
 }
 
+int helios_set_tp_elements(helios_ctx* c, int n_elements, int order, int ratio_form) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_atmo) return fail(c, HELIOS_ESTATE, "set_tp_elements: call helios_set_atmosphere first");
+    if (n_elements < 1 || n_elements > 16 || order < 1 || order > 4)
+        return fail(c, HELIOS_EINVAL, "set_tp_elements: n_elements %d (1..16), order %d (1..4)", n_elements, order);
+    CU_TRY(c, cudaSetDevice(c->device));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    c->tp_order = order; c->tp_ratio = ratio_form ? 1 : 0; c->NT = n_elements * order + 1;
+    CU_TRY(c, build_tp(c, n_elements, order));
+    c->cap_B = 0;    // the parameter staging buffer depends on P
+    return HELIOS_OK;
+}
+
+int helios_set_extras(helios_ctx* c, unsigned flags) {
+    if (!c) return HELIOS_EINVAL;
+    if (flags & ~(HELIOS_EXTRA_DISTANCE | HELIOS_EXTRA_ERROR_INFLATION | HELIOS_EXTRA_GREY_CLOUD))
+        return fail(c, HELIOS_EINVAL, "set_extras: unknown flag in 0x%x", flags);
+    c->extras = flags;
+    c->n_extra = ((flags & HELIOS_EXTRA_DISTANCE) ? 1 : 0) + ((flags & HELIOS_EXTRA_ERROR_INFLATION) ? 1 : 0) +
+                 ((flags & HELIOS_EXTRA_GREY_CLOUD) ? 3 : 0);
+    c->cap_B = 0;
+    return HELIOS_OK;
+}
+
+int helios_get_n_params(const helios_ctx* c, int* out) {
+    if (!c || !out || !c->have_atmo) return HELIOS_EINVAL;
+    *out = n_params(c);
+    return HELIOS_OK;
+}
+
+int helios_teff_batch(helios_ctx* c, int B, const double* params, double nu_a, double nu_b, double* teff_out) {
+    int rc = check_ready(c, B, params, false, false);
+    if (rc) return rc;
+    if (!teff_out) return fail(c, HELIOS_EINVAL, "teff_out is NULL");
+    const double nu_first = c->nu0, nu_last = c->nu0 + c->dnu * (c->nNu - 1);
+    if (!(nu_b > nu_a) || nu_a < nu_first - 1e-9 * c->dnu || nu_b > nu_last + 1e-9 * c->dnu)
+        return fail(c, HELIOS_EINVAL, "teff: window [%g, %g] outside the grid [%g, %g]", nu_a, nu_b, nu_first, nu_last);
+    CU_TRY(c, cudaSetDevice(c->device));
+    if ((rc = helios_reserve(c, B))) return rc;
+    c->n_models += B;
+    if ((rc = run_flux(c, B, params, c->d_flux, c->flux_stride, /*unit_scale=*/1))) return rc;
+    TeffArgs ta{c->nNu, c->nu0, c->dnu, std::fmax(nu_a, nu_first), std::fmin(nu_b, nu_last), c->d_flux, c->flux_stride,
+                c->d_flag, teff_out};
+    k_teff<<<B, 256, 0, c->stream>>>(ta);
+    c->n_launches += 1;
+    CU_TRY(c, cudaGetLastError());
+    if (c->opt_timing) { c->ev_has_obs[c->timed_calls % helios_ctx::kTimingRing] = false; c->timed_calls++; }
+    return HELIOS_OK;
+}
+
 int helios_forward_batch_host(helios_ctx* c, int B, const double* params_host, float* spectra_host, double* logl_host) {
     int rc = check_ready(c, B, params_host, true, logl_host != nullptr);
     if (rc) return rc;
     if (!spectra_host && !logl_host) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
     CU_TRY(c, cudaSetDevice(c->device));
     if ((rc = helios_reserve(c, B))) return rc;
-    const size_t P = 2 + c->K + c->S;
+    const size_t P = n_params(c);
     CU_TRY(c, cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * P, cudaMemcpyHostToDevice, c->stream));
     rc = helios_forward_batch(c, B, c->d_params_stage, spectra_host ? c->d_spectra_stage : nullptr,
                               logl_host ? c->d_logl_stage : nullptr);

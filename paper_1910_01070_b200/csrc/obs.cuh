@@ -85,6 +85,8 @@ struct ObsApplyArgs {
     double logl_const;        // -1/2 sum_j ln(2 pi sigma_j^2)
     float* spectra;           // DEVICE [B][J] or nullptr
     double* logl;             // DEVICE [B] or nullptr
+    const double* var;        // DEVICE [J]  sigma_j^2          } error inflation (Eq. 22-23): both non-null,
+    const double* addvar;     // DEVICE [B]  10^epsilon of each model } s_j^2 = var_j + addvar_b
     double* partial;          // DEVICE [B][n_chunks] chi-square of each bin chunk (workspace)
     unsigned* arrived;        // DEVICE [B] chunks finished per model; zero between launches (workspace)
 };
@@ -105,6 +107,7 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
     constexpr int kPerWarp = kObsBinsPerCta / (kObsThreads / 32);
     const bool bad = a.model_flag[b] != 0;
     const float* F = a.flux + (size_t)b * a.flux_stride;
+    const double add = a.addvar ? a.addvar[b] : 0.0;
     double chi2 = 0.0;
     const int j0 = chunk * kObsBinsPerCta + warp * kPerWarp;
 #pragma unroll 2
@@ -126,8 +129,13 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
             if (bad) acc = __int_as_float(0x7fc00000);
             if (a.spectra) a.spectra[(size_t)b * a.J + j] = acc;
             if (a.logl) {
-                double r = a.obs[j] - (double)acc;
-                chi2 += r * r * a.inv2var[j];
+                const double r = a.obs[j] - (double)acc;
+                if (a.addvar) {                       // Eq. 23: the normalisation depends on the model too
+                    const double s2 = a.var[j] + add;
+                    chi2 += r * r / (2.0 * s2) + 0.5 * log(2.0 * kPi * s2);
+                } else {
+                    chi2 += r * r * a.inv2var[j];
+                }
             }
         }
     }
@@ -144,9 +152,49 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
             __threadfence();
             double t = 0.0;
             for (int c = 0; c < n_chunks; ++c) t += __ldcg(&a.partial[(size_t)b * n_chunks + c]);
-            a.logl[b] = bad ? -CUDART_INF : a.logl_const - t;
+            a.logl[b] = bad ? -CUDART_INF : (a.addvar ? -t : a.logl_const - t);
             a.arrived[b] = 0;
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Effective temperature (Sect. 2.6): F_tot = integral of F+ over [nu_a, nu_b]
+// (trapezoid on the grid with interpolated end points = sum_i F_i * integral of the hat function of
+// grid point i over the window), T_eff = (F_tot / sigma_SB)^(1/4).  One CTA per model, fp64 sums
+// combined in a fixed order.
+// ---------------------------------------------------------------------------------------
+struct TeffArgs {
+    int nNu;
+    double nu0, dnu, nu_a, nu_b;
+    const float* flux;        // DEVICE [B][flux_stride]  F+ (prep ran with unit_scale)
+    long long flux_stride;
+    const int* model_flag;
+    double* teff;             // DEVICE [B]
+};
+
+__global__ void __launch_bounds__(256) k_teff(TeffArgs a) {
+    __shared__ double part[256];
+    const int b = blockIdx.x;
+    const float* F = a.flux + (size_t)b * a.flux_stride;
+    int ia = (int)floor((a.nu_a - a.nu0) / a.dnu), ib = (int)ceil((a.nu_b - a.nu0) / a.dnu);
+    ia = max(ia, 0); ib = min(ib, a.nNu - 1);
+    double s = 0.0;
+    for (int i = ia + threadIdx.x; i <= ib; i += 256) {
+        const double nu_i = a.nu0 + a.dnu * i;
+        const double h = (hat_cdf((a.nu_b - nu_i) / a.dnu) - hat_cdf((a.nu_a - nu_i) / a.dnu)) * a.dnu;
+        s += h * (double)F[i];
+    }
+    part[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const double sigma_sb = 2.0 * kPi * kPi * kPi * kPi * kPi * kBoltzmann * kBoltzmann * kBoltzmann * kBoltzmann /
+                                (15.0 * kPlanckH * kPlanckH * kPlanckH * kLightC * kLightC);
+        a.teff[b] = a.model_flag[b] ? CUDART_NAN : pow(part[0] / sigma_sb, 0.25);
     }
 }
 

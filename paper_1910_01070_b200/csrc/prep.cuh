@@ -12,8 +12,14 @@ struct PrepArgs {
     int B, P, K, S, C, L, nT, nP;
     const double* T_grid;     // DEVICE [nT]
     const double* lvl_p_bar;  // DEVICE [L]
-    const int*    lvl_knot;   // DEVICE [L]  element index of the level
-    const double* lvl_xi;     // DEVICE [L]  reference-element coordinate in [0,1]
+    const int*    lvl_elem;   // DEVICE [L]  finite element the level lies in
+    const double* lvl_lw;     // DEVICE [L][kMaxTpNodes]  Lagrange weights of the element's nodes at the level (Eq. 13)
+    int tp_order;             // q: element k owns the temperature parameters k q .. k q + q (0: one isothermal value)
+    int tp_ratio;             // 1: parameters are (T_1, b_2 .. b_N), T_i = b_i T_{i-1}
+    int NT;                   // number of temperature parameters (replaces K in the parameter vector)
+    unsigned extras;          // HELIOS_EXTRA_* flags: extra parameters after the VMRs
+    int unit_scale;           // 1: model_scale = 2 pi (F+ of Eq. 8, for T_eff); 0: 2 pi f flux_const [/ d^2] (Eq. 9)
+    double* model_addvar;     // DEVICE [B]  10^epsilon of Eq. 22 (0 without error inflation)
     const int*    lvl_ip;     // DEVICE [L]  pressure cell
     const double* lvl_u;      // DEVICE [L]  pressure weight in [0,1]
     const int*    lvl_pclamp; // DEVICE [L]  1 if the level pressure is outside the table
@@ -29,9 +35,21 @@ struct PrepArgs {
     unsigned long long* counters;  // [0] clamped pairs, [1] non-finite models
 };
 
-__device__ __forceinline__ double knot_temperature(const double* th_knots, int K, int k, double xi) {
-    if (K == 1) return th_knots[0];
-    return th_knots[k] * (1.0 - xi) + th_knots[k + 1] * xi;
+constexpr int kMaxTpNodes = 5;    // order <= 4
+
+// Eq. 12: T(level) = sum_i T_dof[k q + i] l_i(xi).  In the ratio form the nodal temperatures are the
+// running products T_1 b_2 ... b_j (R28), rebuilt here for the element's q + 1 nodes.
+__device__ __forceinline__ double level_temperature(const double* tpar, int q, int ratio, int k, const double* lw) {
+    if (q == 0) return tpar[0];
+    double T_node = tpar[0];
+    if (ratio) { for (int j = 1; j <= k * q; ++j) T_node *= tpar[j]; }
+    else T_node = tpar[k * q];
+    double T = T_node * lw[0];
+    for (int i = 1; i <= q; ++i) {
+        T_node = ratio ? T_node * tpar[k * q + i] : tpar[k * q + i];
+        T += T_node * lw[i];
+    }
+    return T;
 }
 
 __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
@@ -45,7 +63,11 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     float* rec = a.rec + ((size_t)b * a.L + l) * a.rec_floats;
     if (l == 0) {
         a.model_flag[b] = finite ? 0 : 1;
-        a.model_scale[b] = finite ? (float)(th[1] * a.flux_const * 2.0 * kPi) : 0.0f;
+        double scale = a.unit_scale ? 1.0 : th[1] * a.flux_const;
+        int ie = 2 + a.NT + a.S;
+        if (a.extras & 1u) { if (!a.unit_scale) scale /= th[ie] * th[ie]; ++ie; }     // distance, Eq. 9
+        a.model_addvar[b] = (a.extras & 2u) ? pow(10.0, th[ie]) : 0.0;                 // error inflation, Eq. 22
+        a.model_scale[b] = finite ? (float)(scale * 2.0 * kPi) : 0.0f;
         if (!finite) atomicAdd(&a.counters[1], 1ULL);
     }
     if (!finite) {
@@ -55,10 +77,10 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     }
 
     const double g = pow(10.0, th[0]);
-    const double* knots = th + 2;
-    const double* lvmr = th + 2 + a.K;
+    const double* tpar = th + 2;
+    const double* lvmr = th + 2 + a.NT;
 
-    const double T = knot_temperature(knots, a.K, a.lvl_knot[l], a.lvl_xi[l]);
+    const double T = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l], a.lvl_lw + (size_t)l * kMaxTpNodes);
     const double p = a.lvl_p_bar[l];
 
     // temperature cell: largest iT with T_grid[iT] <= T, clamped to [0, nT-2]
@@ -117,15 +139,25 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
         rec[o++] = a_hi;
         rec[o++] = (float)(a - (double)a_hi);
     }
-    double hdz = 0.0;
+    double hdz = 0.0, dtc = 0.0;
     if (l + 1 < a.L) {
-        double T_up = knot_temperature(knots, a.K, a.lvl_knot[l + 1], a.lvl_xi[l + 1]);
+        double T_up = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l + 1],
+                                        a.lvl_lw + (size_t)(l + 1) * kMaxTpNodes);
         double dz = kBoltzmann * 0.5 * (T + T_up) / (a.mmw * kAtomicMass * g) * a.lvl_lnratio[l];
         hdz = 0.5 * dz;
+        if (a.extras & 4u) {
+            // grey cloud (App. B, R29): tau_c spread uniformly in pressure over [p_top, p_top (1 + phi)];
+            // the layer between levels l and l+1 gets the share of its pressure overlap
+            const double* cp = th + 2 + a.NT + a.S + ((a.extras & 1u) ? 1 : 0) + ((a.extras & 2u) ? 1 : 0);
+            const double tau_c = pow(10.0, cp[0]), p_top_c = pow(10.0, cp[1]), p_bot_c = p_top_c * (1.0 + pow(10.0, cp[2]));
+            const double hi = fmin(p, p_bot_c), lo = fmax(a.lvl_p_bar[l + 1], p_top_c);
+            if (hi > lo) dtc = tau_c * (hi - lo) / (p_bot_c - p_top_c);
+        }
     }
     rec[o++] = (float)hdz;
     if (!a.slab_layout) rec[o++] = __int_as_float(iT * a.nP + a.lvl_ip[l]);
     rec[o++] = __int_as_float(iT);
+    rec[o++] = (float)dtc;
     while (o < a.rec_floats) rec[o++] = 0.0f;
 }
 

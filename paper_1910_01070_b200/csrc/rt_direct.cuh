@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
     float J[A];
 #pragma unroll
     for (int k = 0; k < A; ++k) J[k] = 0.0f;
-    float chi_prev = 0.0f, S_prev = 0.0f, hdz_prev = 0.0f;
+    float chi_prev = 0.0f, S_prev = 0.0f, hdz_prev = 0.0f, dtc_prev = 0.0f;
 
     for (int l = 0; l < a.L; ++l) {
         const float* r = srec + l * a.rec_floats;
@@ -75,14 +75,14 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
         const float E = planck_E(r[PA], r[PA + 1], nu, nu_lo);
         const float Sl = planck_from_E(c1nu3, E);
         if (l > 0) {
-            const float dtau = (chi + chi_prev) * hdz_prev;
+            const float dtau = fmaf(chi + chi_prev, hdz_prev, dtc_prev);
             const float dS = S_prev - Sl;
             const float q = dS * rcp_approx(dtau);
 #pragma unroll
             for (int k = 0; k < A; ++k)
                 sc_update(J[k], dtau, q, dS, a.ang.c_exp[k], a.ang.inv_mu[k], a.ang.mu[k]);
         }
-        chi_prev = chi; S_prev = Sl; hdz_prev = r[PA + 2];
+        chi_prev = chi; S_prev = Sl; hdz_prev = r[PA + 2]; dtc_prev = r[PA + 5];
     }
     // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = J_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
     float acc = S_prev * a.ang.wmu_sum;

@@ -245,7 +245,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 #pragma unroll
     for (int k = 0; k < A; ++k) H[k] = make_float2(0.0f, 0.0f);
     float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
-    float hdz_prev = 0.0f;
+    float hdz_prev = 0.0f, dtc_prev = 0.0f;
     float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
     int released = 0, cur_iT = -2, prev_lo = -1;
 
@@ -306,13 +306,13 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             const float2 om = __fadd2_rn(bc2(1.0f), neg2(E));
             const float2 Sl = __fmul2_rn(c1nu3, __fmul2_rn(E, make_float2(rcp_approx(om.x), rcp_approx(om.y))));
             if (l > 0) {
-                const float2 dtau = __fmul2_rn(__fadd2_rn(chi, chi_prev), bc2(hdz_prev));
+                const float2 dtau = __ffma2_rn(__fadd2_rn(chi, chi_prev), bc2(hdz_prev), bc2(dtc_prev));
                 const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
                 const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
                 const float2 ndtau = neg2(dtau);
                 all_angles<A>(H, dtau, ndtau, q, dS, std::make_integer_sequence<int, A>{});
             }
-            chi_prev = chi; S_prev = Sl; hdz_prev = r2.x;
+            chi_prev = chi; S_prev = Sl; hdz_prev = r2.x; dtc_prev = r2.z;
         }
         if (a.S > 0 && seg + 1 < a.n_seg) {
             // slots holding loads older than the next segment's are free for the producer
