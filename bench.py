@@ -30,7 +30,7 @@ ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 HBM_NOMINAL_GBS = 8000.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
 # ncu --set full capture summarised in profiles/ (None until captured for this workload).
-NCU_TRAFFIC_BYTES = {2: 216861696 + 15771648}   # profiles/r01_k_rt_slab_ncu_full.txt
+NCU_TRAFFIC_BYTES = {2: 216309248 + 16101120}   # profiles/r01_k_rt_slab_ncu_full.txt
 
 
 def algorithmic_ops(cfg):
