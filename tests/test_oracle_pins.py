@@ -525,3 +525,32 @@ def test_clamp_count(oracle):
     p = oracle.level_pressures(wl.cfg.n_levels, 300.0, 1e-3)
     T = oracle.temperature_profile(p, params[0, 2:4], 300.0, 1e-3)
     assert r["n_clamped"] == int(np.sum(T > 2000.0))
+
+
+def test_oracle_is_clean_under_ubsan(tmp_path):
+    """The oracle built with -fsanitize=undefined -fno-sanitize-recover runs the tiny workload
+    (and the NEXT rows) without tripping: no signed overflow, bad shifts, misaligned or
+    out-of-bounds accesses the compiler can see, NaN->int conversions ..."""
+    import os, subprocess, sys, textwrap
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    so = tmp_path / "liboracle_ubsan.so"
+    r = subprocess.run(["gcc", "-O1", "-g", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-fsanitize=undefined",
+                        "-fno-sanitize-recover=undefined", "-o", str(so), os.path.join(root, "oracle", "helios_oracle.c"),
+                        "-lm"], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip("gcc has no usable UBSan runtime here: " + r.stderr[-200:])
+    code = textwrap.dedent(f"""
+        import sys; sys.path.insert(0, {root!r})
+        import numpy as np, oracle.binding as ob
+        ob._SO = {str(so)!r}; ob.build = lambda force=False: ob._SO
+        import oracle, workloads
+        wl = workloads.make_workload(0)
+        r = oracle.forward_workload(wl, want_flux=True, teff_range=(4000.0, 4999.0))
+        p = np.concatenate([wl.params[0], [2.0, 4.0, -1.0, -1.0, 0.0]])[None, :]
+        r2 = oracle.forward_workload(wl, params=p, extras=7)
+        assert np.isfinite(r["logl"]).all() and np.isfinite(r2["logl"]).all()
+        print("ok")
+    """)
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0 and "ok" in out.stdout, out.stderr[-2000:]
+    assert "runtime error" not in out.stderr
