@@ -231,7 +231,7 @@ def run_gpu(args):
     # re-reads them from HBM.  Smaller tables (configs[0], [1]) would stay L2-resident from one step to
     # the next: then each step is timed on its own and 256 MiB are written between steps to flush L2.
     table_bytes = wl.sigma.nbytes + wl.cia.nbytes
-    flush_l2 = table_bytes < 1.5 * 126e6
+    flush_l2 = table_bytes < 1.5 * 126e6 and not os.environ.get("HELIOS_BENCH_NOFLUSH")
     scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush_l2 else None
 
     def timed(fn, steps, sampler=None):
