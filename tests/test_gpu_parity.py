@@ -274,3 +274,34 @@ def test_error_codes(torch_cuda, wl0):
     torch.cuda.synchronize()
     assert torch.isfinite(spec).all()
     h.close()
+
+
+def test_auto_falls_back_to_the_direct_kernel_when_planes_do_not_fit(torch_cuda, oracle):
+    """40 species x 30 temperature nodes: one table plane would need 307 KB of shared memory, so the
+    automatic choice must be the direct kernel, and forcing the staged kernel must fail loudly."""
+    import paper_1910_01070_b200 as pkg
+    torch = torch_cuda
+    rng = np.random.default_rng(5)
+    S, nT, nP, nNu, L, K, A, B = 40, 30, 3, 200, 15, 2, 2, 9
+    T_grid = np.linspace(200.0, 3200.0, nT); lp_grid = np.array([-4.0, 0.0, 3.0])
+    sigma = (10.0 ** rng.uniform(-27, -22, (S, nT, nP, nNu))).astype(np.float32)
+    edges = np.linspace(3000.0, 3000.0 + nNu - 1, 11)
+    params = np.column_stack([rng.uniform(4, 5.5, B), rng.uniform(0.5, 2, B),
+                              -np.sort(-rng.uniform(500, 2800, (B, K)), axis=1), rng.uniform(-8, -3, (B, S))])
+    ref = oracle.forward(T_grid, lp_grid, 3000.0, 1.0, sigma, None, L, 100.0, 1e-3, K, A, 2.3, 0.17, 1.0,
+                         edges, None, None, None, params, want_flux=True, want_logl=False)
+    h = pkg.Helios(0)
+    h.load_opacity(T_grid, lp_grid, 3000.0, 1.0, sigma, None)
+    h.set_atmosphere(L, 100.0, 1e-3, K, A, 2.3, 0.17, 1.0)
+    h.set_observation(edges)
+    p = torch.as_tensor(params, device="cuda:0")
+    spec, _ = h.forward_batch(p, want_logl=False)
+    flux = h.forward_highres(p)
+    torch.cuda.synchronize()
+    assert _relerr(flux.cpu().numpy().astype(np.float64), ref["flux_hr"]) <= TOL_FLUX
+    assert _relerr(spec.cpu().numpy().astype(np.float64), ref["spectra"]) <= TOL_FLUX
+    h.set_kernel(2)
+    with pytest.raises(pkg.HeliosError) as ei:
+        h.forward_highres(p)
+    assert ei.value.code == pkg.HELIOS_EINVAL
+    h.close()
