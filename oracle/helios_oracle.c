@@ -16,8 +16,11 @@
  * table in DESIGN.md "Oracle pins".  What CANNOT be pinned is agreement with
  * the ORIGINAL Helios-r2 code on the four points the paper never prints
  * (interpolant of sigma, optical-depth formula, convolution normalisation,
- * binning rule: DESIGN.md readings R1, R5, R15, R17) -- "parity unpinned" for
- * those readings; the arithmetic given the readings is pinned.
+ * binning rule: DESIGN.md readings R1, R5, R15, R17) and, for the rows added
+ * after the hot path (ratio form of the T-p parameters, grey-cloud geometry,
+ * T_eff quadrature: R28, R29, R30) -- "parity unpinned" for those readings;
+ * the arithmetic given the readings is pinned (tests/test_oracle_pins.py,
+ * tests/test_oracle_next.py).
  *
  * Precision: all arithmetic in fp64; the cross-section tables are the same
  * fp32 values the GPU gets, promoted to double.
