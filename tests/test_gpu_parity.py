@@ -305,3 +305,52 @@ def test_auto_falls_back_to_the_direct_kernel_when_planes_do_not_fit(torch_cuda,
         h.forward_highres(p)
     assert ei.value.code == pkg.HELIOS_EINVAL
     h.close()
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_shapes_staged_kernel(torch_cuda, oracle, seed):
+    """Random table / atmosphere shapes through the staged kernel: pressure grids denser than the
+    levels (segments that skip table cells, two new planes per segment), two-node grids, two levels,
+    one to eight angles, batches that do not fill a CTA, ring wrap-around with many planes."""
+    import paper_1910_01070_b200 as pkg
+    torch = torch_cuda
+    rng = np.random.default_rng(1000 + seed)
+    S = int(rng.integers(0, 6)); C = int(rng.integers(0, 3))
+    if S + C == 0:
+        S = 1
+    nT = int(rng.integers(2, 12)); nP = int(rng.choice([2, 3, 9, 40])); nNu = int(rng.integers(60, 300))
+    L = int(rng.choice([2, 3, 7, 30, 90])); A = int(rng.integers(1, 9)); K = int(rng.integers(1, 5))
+    B = int(rng.choice([1, 5, 17, 33]))
+    T_grid = np.sort(rng.uniform(200.0, 3200.0, nT)); T_grid[0] = 200.0; T_grid[-1] = 3200.0
+    T_grid = np.unique(np.round(T_grid, 3))
+    nT = len(T_grid)
+    if nT < 2:
+        T_grid = np.array([200.0, 3200.0]); nT = 2
+    lp_grid = np.linspace(-4.5, 2.5, nP) + (rng.uniform(-0.05, 0.05, nP) if nP > 2 else 0.0)
+    lp_grid = np.sort(lp_grid)
+    sigma = (10.0 ** rng.uniform(-27, -21, (S, nT, nP, nNu))).astype(np.float32)
+    cia = (10.0 ** rng.uniform(-9, -7, (C, nT, nNu))).astype(np.float32) if C else None
+    nu0, dnu = 3000.0, 0.7
+    edges = np.linspace(nu0, nu0 + dnu * (nNu - 1), 7)
+    inst = np.full(nNu, 2.0)
+    params = np.column_stack([rng.uniform(4, 5.5, B), rng.uniform(0.5, 2, B),
+                              -np.sort(-rng.uniform(300, 3000, (B, K)), axis=1), rng.uniform(-8, -2, (B, S))])
+    obs = np.full(6, 1e4); err = np.full(6, 1e3)
+    ref = oracle.forward(T_grid, lp_grid, nu0, dnu, sigma, cia, L, 200.0, 2e-4, K, A, 2.3, 0.17, 1.0,
+                         edges, obs, err, inst, params, want_flux=True)
+    h = pkg.Helios(0)
+    h.load_opacity(T_grid, lp_grid, nu0, dnu, sigma, cia)
+    h.set_atmosphere(L, 200.0, 2e-4, K, A, 2.3, 0.17, 1.0)
+    h.set_observation(edges, obs, err, inst)
+    h.set_kernel(2)
+    p = torch.as_tensor(params, device="cuda:0")
+    spec, logl = h.forward_batch(p)
+    flux = h.forward_highres(p)
+    torch.cuda.synchronize()
+    st = h.stats()
+    h.close()
+    shape = dict(S=S, C=C, nT=nT, nP=nP, nNu=nNu, L=L, A=A, K=K, B=B)
+    assert _relerr(flux.cpu().numpy().astype(np.float64), ref["flux_hr"]) <= TOL_FLUX, shape
+    assert _relerr(spec.cpu().numpy().astype(np.float64), ref["spectra"]) <= TOL_FLUX, shape
+    assert np.max(np.abs(logl.cpu().numpy() - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4, shape
+    assert st["n_clamped"] == 2 * ref["n_clamped"], shape
