@@ -531,9 +531,16 @@ static SlabPlan plan_slab(const helios_ctx* c, int B) {
     SlabPlan none;
     if (c->opt_kernel == 1 || !c->have_tmaps) return none;
     // models per CTA (measured on B200, configs 1-3): 24 warps hide latency best while the state fits
-    // 72 registers (<= 4 angles); 16 otherwise; 8 for batches too small to fill 16-model groups
+    // 72 registers (<= 4 angles) and the batch fills 24-model groups; 16 otherwise; 8 for B < 16
     int nw = c->opt_models_per_cta;
-    if (nw == 0) nw = B < 16 ? 8 : (c->A <= 4 && B >= 128 ? 24 : 16);
+    if (nw == 0) {
+        if (B < 16) nw = 8;
+        else if (c->A > 4) nw = 16;
+        else {      // padded model slots, weighted by the measured per-model efficiency of the two variants
+            const double cost24 = (double)((B + 23) / 24 * 24), cost16 = (double)((B + 15) / 16 * 16) / 0.92;
+            nw = cost24 <= cost16 ? 24 : 16;
+        }
+    }
     return slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, nw, c->smem_optin, c->smem_sm);
 }
 
