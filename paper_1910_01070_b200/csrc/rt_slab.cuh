@@ -377,8 +377,14 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
 template <int A, int NW, int MINB>
 inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, size_t smem,
                                     cudaStream_t stream) {
-    cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    static size_t configured[64] = {};   // per kernel instance and device; setting it again is harmless, so no lock
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || smem > configured[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) configured[dev] = smem;
+    }
     const dim3 grid((a.B + NW - 1) / NW, (a.nNu + kSlabTile - 1) / kSlabTile);
     k_rt_slab<A, NW, MINB><<<grid, (NW + 1) * 32, smem, stream>>>(tms, tmc, a);
     return cudaGetLastError();
