@@ -1,0 +1,52 @@
+"""Mutation check of the oracle's whole-path driver (`oracle_forward_ext`) and of `oracle_convolve`.
+
+Round 1's review found that seven one-token wiring mistakes in the driver passed every CPU pin,
+because all whole-path pins used grey / single-species / pressure-independent tables.  Each mutant
+below is applied to a scratch copy of oracle/helios_oracle.c; the pins named beside it must FAIL on
+the mutant (and pass on the original, which the normal run of those tests shows).  `-m "not gpu"`.
+"""
+import os
+import shutil
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+BRUTE = "test_whole_path_brute_force_tiny_nongrey"
+MUTANTS = {
+    # name: (original text, mutated text, pin that must fail)
+    "M1_h2_he_swapped": ("oracle_chi_level(S, x, sig, C, x_h2, x_he, alp,",
+                         "oracle_chi_level(S, x, sig, C, x_he, x_h2, alp,", BRUTE),
+    "M2_cia_pair_offset_dropped": ("oracle_interp_cia(cia + (size_t)c * nT * nNu, nT, T_grid, nNu, T[l], alp[c]);",
+                                   "oracle_interp_cia(cia, nT, T_grid, nNu, T[l], alp[c]);", BRUTE),
+    "M4_cia_at_bottom_temperature": ("oracle_interp_cia(cia + (size_t)c * nT * nNu, nT, T_grid, nNu, T[l], alp[c]);",
+                                     "oracle_interp_cia(cia + (size_t)c * nT * nNu, nT, T_grid, nNu, T[0], alp[c]);", BRUTE),
+    "M5_sigma_at_bottom_pressure": ("nNu, T[l], log10(p_bar[l]), sig[s], &cl);",
+                                    "nNu, T[l], log10(p_bar[0]), sig[s], &cl);", BRUTE),
+    "M6_species_offset_dropped": ("oracle_interp_sigma(sigma + (size_t)s * nT * nP * nNu, nT,",
+                                  "oracle_interp_sigma(sigma, nT,", BRUTE),
+    "M7_inst_sigma_one_point_off": ("double sg = inst_sigma ? inst_sigma[k] : 0.0;\n        if (sg <= 0.0) { Fd[k]",
+                                    "double sg = inst_sigma ? inst_sigma[k > 0 ? k - 1 : 0] : 0.0;\n        if (sg <= 0.0) { Fd[k]",
+                                    "test_convolve_closed_forms"),
+    "M17_dtau_column_of_neighbour_nu": ("dcol[l] = dtau[(size_t)l * nNu + k];",
+                                        "dcol[l] = dtau[(size_t)l * nNu + (k > 0 ? k - 1 : 0)];", BRUTE),
+    "M18_density_at_bottom_temperature": ("oracle_number_density(p_bar[l], T[l]), nNu, chi",
+                                          "oracle_number_density(p_bar[l], T[0]), nNu, chi", BRUTE),
+    "M21_trapezoid_uses_one_level": ("chi + (size_t)(l + 1) * nNu, dz,", "chi + (size_t)(l) * nNu, dz,", BRUTE),
+}
+
+
+@pytest.mark.parametrize("name", sorted(MUTANTS))
+def test_mutant_is_killed(name, tmp_path):
+    old, new, pin = MUTANTS[name]
+    src = open(os.path.join(ROOT, "oracle", "helios_oracle.c")).read()
+    assert src.count(old) == 1, f"{name}: the driver changed; update the mutant"
+    for sub in ("oracle", "workloads", "tests"):
+        shutil.copytree(os.path.join(ROOT, sub), tmp_path / sub,
+                        ignore=shutil.ignore_patterns("*.so", "__pycache__", "test_oracle_mutants.py"))
+    (tmp_path / "oracle" / "helios_oracle.c").write_text(src.replace(old, new))
+    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_oracle_pins.py", "-q", "-x", "-k", pin,
+                        "-p", "no:cacheprovider"], cwd=tmp_path, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 1 and "failed" in r.stdout, f"mutant {name} survived {pin}:\n{r.stdout[-1500:]}"

@@ -349,6 +349,11 @@ def test_convolve_closed_forms(oracle):
     sig2 = np.where(np.arange(n) < 200, 1.0, 4.0)
     out2 = oracle.convolve(nu0, dnu, spike, sig2)
     assert out2[190] == pytest.approx(math.exp(-25.0 / 2.0) / np.exp(-(dnu * np.arange(-10, 11)) ** 2 / 2.0).sum(), rel=1e-12)
+    # ... probed right at the step, where a one-point shift of the sigma index changes the answer:
+    # point 199 still has sigma = 1 (window +-10 points), point 200 is the first with sigma = 4 (+-40 points)
+    assert out2[199] == pytest.approx(math.exp(-0.25 / 2.0) / np.exp(-(dnu * np.arange(-10, 11)) ** 2 / 2.0).sum(), rel=1e-12)
+    assert out2[200] == pytest.approx(1.0 / np.exp(-(dnu * np.arange(-40, 41)) ** 2 / 32.0).sum(), rel=1e-12)
+    assert out2[201] == pytest.approx(math.exp(-0.25 / 32.0) / np.exp(-(dnu * np.arange(-40, 41)) ** 2 / 32.0).sum(), rel=1e-12)
 
 
 # --------------------------------------------------------------------------
@@ -554,3 +559,141 @@ def test_oracle_is_clean_under_ubsan(tmp_path):
     out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
     assert out.returncode == 0 and "ok" in out.stdout, out.stderr[-2000:]
     assert "runtime error" not in out.stderr
+
+
+# --------------------------------------------------------------------------
+# Whole path, brute force on a tiny NON-grey case  (P4 + P6, north_star's fifth closed form:
+# "brute-force trapezoid tau on tiny inputs").  Everything between the parameter vector and the
+# per-wavenumber (S, dtau) columns is recomputed here by hand in numpy from the paper's statements
+# (PAPER.md:55 levels, :174-190 first-order elements, :484 H2/He fill, :241 interpolation to the level
+# (T, p), :127/:133 species + H2-H2/H2-He CIA, :239 optical depths / DESIGN.md R5), with the table values
+# taken from its ANALYTIC form and from scipy's RegularGridInterpolator, never from the oracle.  The
+# table depends on species, T, p and nu, both CIA pairs are non-zero and differ, He/H2 != 1, the
+# profile is not isothermal: every index the driver `oracle_forward_ext` passes along (species offset,
+# CIA pair offset, level temperature, level pressure, wavenumber column, x_H2 / x_He) changes the result.
+# Mutants of the driver this test kills are listed in DESIGN.md section 3.
+# --------------------------------------------------------------------------
+def _nongrey_tiny_case():
+    T_grid = np.array([300.0, 900.0, 1400.0, 2600.0])
+    lp_grid = np.array([-3.0, -0.5, 1.0, 2.5])
+    nu0, dnu, nNu = 1500.0, 1750.0, 3
+    # sigma_s(nu; T, lp) = a + b T + c lp + d T lp  (exactly bilinear; different per species and per nu)
+    coef = np.array([  # [S][nNu][4]
+        [[4.0e-23, 1.5e-26, 6.0e-24, 2.0e-27], [9.0e-24, 4.0e-27, -1.0e-24, 1.0e-27], [3.0e-22, -3.0e-26, 3.0e-23, 5.0e-27]],
+        [[7.0e-22, -1.0e-25, 1.0e-22, -2.0e-26], [3.0e-23, 2.0e-26, 5.0e-24, -1.0e-27], [5.0e-24, 6.0e-27, 1.0e-24, 5.0e-28]],
+    ])
+    TT, PP = np.meshgrid(T_grid, lp_grid, indexing="ij")
+    sigma = np.empty((2, 4, 4, nNu), np.float32)
+    for s in range(2):
+        for k in range(nNu):
+            a, b, c, d = coef[s, k]
+            sigma[s, :, :, k] = a + b * TT + c * PP + d * TT * PP
+    assert sigma.min() > 0.0
+    # alpha_c(nu; T) = a + b T, cm^-1 amagat^-2; pair 0 = H2-H2, pair 1 = H2-He
+    ccoef = np.array([[[2.0e-6, 3.0e-9], [6.0e-7, -1.0e-10], [1.0e-6, 1.0e-9]],
+                      [[9.0e-6, -2.0e-9], [2.0e-6, 4.0e-9], [4.0e-7, 2.0e-10]]])
+    cia = np.empty((2, 4, nNu), np.float32)
+    for c in range(2):
+        for k in range(nNu):
+            cia[c, :, k] = ccoef[c, k, 0] + ccoef[c, k, 1] * T_grid
+    return dict(T_grid=T_grid, lp_grid=lp_grid, nu0=nu0, dnu=dnu, nNu=nNu, coef=coef, ccoef=ccoef,
+                sigma=sigma, cia=cia)
+
+
+def _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he_to_h2, analytic):
+    """(S_l(nu), dtau_l(nu)) from the paper's statements; `analytic` picks the analytic table or
+    scipy's multilinear interpolation of the stored fp32 nodes."""
+    from scipy.interpolate import RegularGridInterpolator
+    nu = case["nu0"] + case["dnu"] * np.arange(case["nNu"])
+    lev = np.arange(L)
+    lp = math.log10(p_bot) + (math.log10(p_top) - math.log10(p_bot)) * lev / (L - 1)      # PAPER.md:55
+    p_cgs = 10.0 ** lp * 1e6
+    K = len(knots)
+    lp_knots = np.linspace(math.log10(p_bot), math.log10(p_top), K)
+    T = np.interp(-lp, -lp_knots, knots)                       # linear in log p between the nodes (first-order elements)
+    x = 10.0 ** np.asarray(log_vmr)
+    x_bg = 1.0 - x.sum()
+    x_h2, x_he = x_bg / (1.0 + he_to_h2), x_bg * he_to_h2 / (1.0 + he_to_h2)      # PAPER.md:484
+    n = p_cgs / (KB * T)
+    amagat = n / (1.01325e6 / (KB * 273.15))
+    chi = np.zeros((L, case["nNu"]))
+    for l in range(L):
+        for k in range(case["nNu"]):
+            if analytic:
+                sig = [c[0] + c[1] * T[l] + c[2] * lp[l] + c[3] * T[l] * lp[l] for c in case["coef"][:, k]]
+                alp = [c[0] + c[1] * T[l] for c in case["ccoef"][:, k]]
+            else:
+                sig = [RegularGridInterpolator((case["T_grid"], case["lp_grid"]), case["sigma"][s, :, :, k].astype(np.float64))([[T[l], lp[l]]])[0]
+                       for s in range(2)]
+                alp = [np.interp(T[l], case["T_grid"], case["cia"][c, :, k].astype(np.float64)) for c in range(2)]
+            chi[l, k] = n[l] * (x[0] * sig[0] + x[1] * sig[1]) \
+                + amagat[l] ** 2 * x_h2 * (x_h2 * alp[0] + x_he * alp[1])           # PAPER.md:127, 133; R4
+    g = 10.0 ** logg
+    dz = KB * 0.5 * (T[:-1] + T[1:]) / (mmw * MU * g) * np.log(p_cgs[:-1] / p_cgs[1:])   # hydrostatic, R5
+    dtau = 0.5 * (chi[:-1] + chi[1:]) * dz[:, None]                                 # trapezoid, R5
+    S = 2 * H * C * C * nu[None, :] ** 3 / np.expm1(C2 * nu[None, :] / T[:, None])   # Eq. 2
+    return T, S, dtau
+
+
+def test_whole_path_brute_force_tiny_nongrey(oracle):
+    case = _nongrey_tiny_case()
+    L, p_bot, p_top, A = 4, 10.0, 1e-2, 3
+    knots = [2100.0, 1300.0, 700.0]
+    logg, f, flux_const, mmw, he = 5.3, 1.3, 0.7, 2.3, 0.4
+    log_vmr = [-3.0, -3.7]
+    params = np.array([[logg, f] + knots + log_vmr])
+    edges = np.array([1500.0, 2800.0, 5000.0])
+    obs = np.array([3.0e4, 2.0e4])
+    err = np.array([2.0e3, 5.0e3])
+    r = oracle.forward(case["T_grid"], case["lp_grid"], case["nu0"], case["dnu"], case["sigma"], case["cia"],
+                       L, p_bot, p_top, len(knots), A, mmw, he, flux_const, edges, obs, err, None, params,
+                       want_flux=True, want_spectra=True, want_logl=True)
+    assert r["n_clamped"] == 0
+    mu, w = np.polynomial.legendre.leggauss(A)
+    mu, w = 0.5 * (mu + 1.0), 0.5 * w
+    for analytic, rtol in ((False, 1e-12), (True, 2e-6)):          # fp32 storage of the nodes: 6e-8 per value
+        T, S, dtau = _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he, analytic)
+        assert len(set(np.searchsorted(case["T_grid"], T))) >= 3    # the levels sit in different T cells
+        assert dtau.min() > 1e-3 and dtau.max() < 10.0              # neither transparent nor opaque everywhere
+        F = np.array([f * flux_const * oracle.flux_one_nu(S[:, k], dtau[:, k], mu, w) for k in range(case["nNu"])])
+        assert np.allclose(r["flux_hr"][0], F, rtol=rtol, atol=0.0)
+    # each ingredient matters at this working point (so the comparison above is not vacuous)
+    T, S, dtau = _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he, True)
+    F = np.array([f * flux_const * oracle.flux_one_nu(S[:, k], dtau[:, k], mu, w) for k in range(case["nNu"])])
+    for what in ("species0", "species1", "cia0", "cia1"):
+        c2 = {k: (v.copy() if isinstance(v, np.ndarray) else v) for k, v in case.items()}
+        if what.startswith("species"):
+            c2["coef"][int(what[-1])] *= 0.0
+        else:
+            c2["ccoef"][int(what[-1])] *= 0.0
+        _, S2, d2 = _by_hand_columns(c2, L, p_bot, p_top, knots, logg, log_vmr, mmw, he, True)
+        F2 = np.array([f * flux_const * oracle.flux_one_nu(S2[:, k], d2[:, k], mu, w) for k in range(case["nNu"])])
+        assert np.max(np.abs(F2 / F - 1.0)) > 1e-3, what
+    # the rest of the driver: O5-O7 on that flux (no instrument profile here), Eq. 19
+    from scipy.stats import norm
+    nu = case["nu0"] + case["dnu"] * np.arange(case["nNu"])
+    M = [np.trapezoid(np.interp(xs, nu, r["flux_hr"][0]), xs) / (xs[-1] - xs[0])
+         for xs in (np.array([1500.0, 2800.0]), np.array([2800.0, 3250.0, 5000.0]))]
+    assert np.allclose(r["spectra"][0], M, rtol=1e-13)
+    assert r["logl"][0] == pytest.approx(np.sum(norm.logpdf(obs, loc=M, scale=err)), rel=1e-12)
+
+
+def test_whole_path_brute_force_many_levels_and_batch(oracle):
+    # same brute force with more levels than table nodes (several levels per cell, every cell of the
+    # grid crossed), A = 2, and three models in one call (a model's columns must not leak into another's)
+    case = _nongrey_tiny_case()
+    L, p_bot, p_top, A = 9, 200.0, 2e-3, 2
+    mmw, he = 2.5, 0.17
+    models = [(5.0, 1.0, [2500.0, 1500.0, 1000.0, 400.0], [-2.5, -4.0]),
+              (4.2, 0.6, [1200.0, 1100.0, 900.0, 850.0], [-5.0, -2.2]),
+              (5.4, 1.9, [2000.0, 800.0, 700.0, 350.0], [-3.3, -3.1])]
+    params = np.array([[m[0], m[1]] + m[2] + m[3] for m in models])
+    r = oracle.forward(case["T_grid"], case["lp_grid"], case["nu0"], case["dnu"], case["sigma"], case["cia"],
+                       L, p_bot, p_top, 4, A, mmw, he, 1.0, np.array([1500.0, 5000.0]), None, None, None, params,
+                       want_flux=True, want_spectra=False, want_logl=False)
+    mu, w = np.polynomial.legendre.leggauss(A)
+    mu, w = 0.5 * (mu + 1.0), 0.5 * w
+    for b, (logg, f, knots, log_vmr) in enumerate(models):
+        T, S, dtau = _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he, False)
+        F = np.array([f * oracle.flux_one_nu(S[:, k], dtau[:, k], mu, w) for k in range(case["nNu"])])
+        assert np.allclose(r["flux_hr"][b], F, rtol=1e-12, atol=0.0)
