@@ -5,8 +5,11 @@
 A "step" is one pass of the whole hot path (profile prep -> interpolate ->
 optical depth -> RT -> convolve/bin/chi-square) over one batch of synthetic
 input, through the C ABI (helios_forward_batch; spectra and logL written).
-Default workload: BASELINE.json configs[2] (JWST-like broadband, B = 256),
-the configuration the "batch >= 256" target of north_star is quoted on.
+Default workload: BASELINE.json configs[3] (high-resolution opacity sampling,
+85 001 wavenumbers x 150 levels x 8 angles, 1.66 GB of tables, B = 1024), the
+largest single-GPU configuration; --config 4 is the likelihood-only stream
+(16 x 256), --config 0..2 the smaller ones, --workload teff the T_eff
+post-processing workload.
 Prints ONE JSON line.
 """
 import argparse
@@ -25,12 +28,14 @@ import numpy as np  # noqa: E402
 
 import workloads  # noqa: E402
 
-# B200: 148 SMs x 128 FP32 lanes x 1.965 GHz (guide unit counts, clocks.max.sm), 1 FMA = 2 flop
-ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# Fallback only (used when helios_measure_peaks is unavailable): 148 SMs x 128 FP32 lanes x 1.965 GHz
+# (guide unit counts, clocks.max.sm), 1 FMA = 2 flop; 16 MUFU results per clock per SM.
+NOMINAL_FMA_PER_CLK_SM, NOMINAL_MUFU_PER_CLK_SM, NOMINAL_SM_MHZ = 128.0, 16.0, 1965.0
 HBM_NOMINAL_GBS = 8000.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
-# ncu --set full capture summarised in profiles/ (None until captured for this workload).
-NCU_TRAFFIC_BYTES = {2: 216309248 + 16101120}   # profiles/r01_k_rt_slab_ncu_full.txt
+# ncu --set full captures summarised in profiles/ (None until captured for this workload).
+NCU_TRAFFIC_BYTES = {2: 216309248 + 16101120,       # profiles/r01_k_rt_slab_ncu_full.txt
+                     3: 1273274000 + 341796864}     # profiles/r01_k_rt_slab_cfg3_ncu_full.txt
 
 
 def algorithmic_ops(cfg):
@@ -121,8 +126,8 @@ def oracle_sample_size(wl, cfg, cores, target_s=15.0):
     return max(1, min(n, cfg.batch))
 
 
-def time_oracle(wl, n_models, repeats=1, min_wall_s=0.0):
-    """The oracle as it stands (never tuned), all host cores, table generation excluded.
+def time_oracle(wl, n_models, repeats=1, min_wall_s=0.0, n_threads=0):
+    """The oracle as it stands (never tuned), all host cores (n_threads = 0) or n_threads, table generation excluded.
     Returns (mean wall seconds of one pass over n_models models, threads).  Passes are repeated
     until `min_wall_s` of work has been timed, so a whole-batch sample that takes only a second
     or two (configs[1], [2]) is still a 10 s measurement."""
@@ -131,27 +136,41 @@ def time_oracle(wl, n_models, repeats=1, min_wall_s=0.0):
     total, passes = 0.0, 0
     while passes < repeats or total < min_wall_s:
         t0 = time.perf_counter()
-        oracle.forward_workload(wl, params=params, want_spectra=True, want_logl=wl.obs is not None)
+        oracle.forward_workload(wl, params=params, want_spectra=True, want_logl=wl.obs is not None, n_threads=n_threads)
         total += time.perf_counter() - t0
         passes += 1
         if passes >= 200:
             break
-    return total / passes, oracle.max_threads()
+    return total / passes, (n_threads if n_threads > 0 else oracle.max_threads())
+
+
+def workload_for(args):
+    """(cfg, workload name).  --workload teff: the T_eff post-processing workload (Sect. 2.6, PAPER.md:223-227;
+    SURVEY.md 8(f) NEXT-3) = helios_teff_batch over 500-10 000 cm^-1 (1-20 micron) on the configs[2] tables and grid."""
+    index = 2 if args.workload == "teff" and args.config < 0 else (3 if args.config < 0 else args.config)
+    cfg = workloads.get_config(index)
+    if args.batch > 0:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, batch=args.batch * cfg.n_calls)
+    name = f"configs[{cfg.index}] {cfg.name}"
+    if args.workload == "teff":
+        name = f"teff: T_eff over 500-10000 cm^-1 on {name}"
+    return cfg, name
 
 
 def run_reference(args):
     """--impl reference: the fp64 CPU oracle on this box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    cfg = workloads.get_config(args.config)
-    wl = workloads.make_workload(args.config, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls)
+    cfg, name = workload_for(args)
+    wl = workloads.make_workload(cfg.index, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls)
     import oracle
     cores = oracle.max_threads()
     # keep the whole --steps K --warmup W run within a few minutes: ~60 s of oracle time in total
     n = oracle_sample_size(wl, cfg, cores, target_s=min(15.0, 60.0 / max(1, args.steps)))
     for _ in range(args.warmup):
-        time_oracle(wl, min(n, cores))
-    t = [time_oracle(wl, n)[0] for _ in range(args.steps)]
+        time_oracle(wl, min(n, cores), n_threads=cores)
+    t = [time_oracle(wl, n, n_threads=cores)[0] for _ in range(args.steps)]
     dt = float(np.mean(t))
     value = n / dt
     sample = f"{n} of {cfg.batch} models of configs[{cfg.index}] per step, all nu/levels/bins"
@@ -159,7 +178,7 @@ def run_reference(args):
         "impl": "reference", "metric": "forward_models_per_s", "value": value, "unit": "models/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "batch_per_step": n, "n_nu": cfg.n_nu,
+        "config": {"workload": name, "batch_per_step": n, "n_nu": cfg.n_nu,
                    "n_levels": cfg.n_levels, "n_species": cfg.n_species, "n_cia": cfg.n_cia,
                    "n_angles": cfg.n_angles, "n_bins": cfg.n_bins},
         "points_per_s": value * cfg.n_nu,
@@ -184,23 +203,29 @@ def run_gpu(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
 
-    cfg = workloads.get_config(args.config)
-    if args.batch > 0:
-        import dataclasses
-        cfg = dataclasses.replace(cfg, batch=args.batch * cfg.n_calls)
+    cfg, wl_name = workload_for(args)
+    teff = args.workload == "teff"
     n_calls = cfg.n_calls                       # configs[4]: 16 back-to-back calls per step
     B_call = cfg.batch // n_calls
-    wl = workloads.make_workload(args.config, batch=cfg.batch, device="cuda")
-    # weak scaling over the batch: every rank evaluates its own cfg.batch models against replicated
-    # tables; rank r draws different parameter vectors.
+    wl = workloads.make_workload(cfg.index, batch=cfg.batch, device="cuda")
+    # replicas: every rank evaluates its own cfg.batch models against replicated tables, no data-path
+    # collective; rank r draws different parameter vectors.
     if rank > 0:
         rng = np.random.default_rng([cfg.seed, rank])
         wl.params = wl.params[rng.permutation(cfg.batch)]
-    want_spec = cfg.spectra_out
+    want_spec = cfg.spectra_out and not teff
 
     h = Helios(local)
     h.setup_workload(wl)
     h.set_kernel(args.kernel, args.models_per_cta)
+    # measured FP32-FMA / MUFU rates of THIS GPU, before the timed region (the roofline denominators)
+    try:
+        pk = h.measure_peaks()
+        peak_src = "measured by helios_measure_peaks on this GPU just before the timed region"
+    except Exception as exc:          # keep the bench alive; say that the peak is nominal
+        pk = {"ffma_per_clk_sm": NOMINAL_FMA_PER_CLK_SM, "ffma2_per_clk_sm": NOMINAL_FMA_PER_CLK_SM,
+              "mufu_per_clk_sm": NOMINAL_MUFU_PER_CLK_SM, "sm_clock_mhz": NOMINAL_SM_MHZ, "n_sms": 148}
+        peak_src = f"nominal fallback ({exc})"
     P = wl.params.shape[1]
     p_dev = torch.as_tensor(wl.params, device=dev)
     spec = torch.empty((cfg.batch, cfg.n_bins), dtype=torch.float32, device=dev) if want_spec else None
@@ -208,18 +233,26 @@ def run_gpu(args):
     p_host = torch.as_tensor(wl.params).pin_memory()
     spec_host = torch.empty((cfg.batch, cfg.n_bins), dtype=torch.float32).pin_memory() if want_spec else None
     logl_host = torch.empty((cfg.batch,), dtype=torch.float64).pin_memory()
+    NU_A, NU_B = 500.0, 10000.0
 
-    from paper_1910_01070_b200 import helios_forward_batch, helios_forward_batch_host
+    from paper_1910_01070_b200 import (helios_forward_batch, helios_forward_batch_host, helios_teff_batch,
+                                       helios_teff_batch_host)
 
     def step_device():
         for c in range(n_calls):
             s = slice(c * B_call, (c + 1) * B_call)
-            helios_forward_batch(h.ctx, p_dev[s], spec[s] if want_spec else None, logl[s])
+            if teff:
+                helios_teff_batch(h.ctx, p_dev[s], NU_A, NU_B, logl[s])
+            else:
+                helios_forward_batch(h.ctx, p_dev[s], spec[s] if want_spec else None, logl[s])
 
     def step_host():
         for c in range(n_calls):
             s = slice(c * B_call, (c + 1) * B_call)
-            helios_forward_batch_host(h.ctx, p_host[s], spec_host[s] if want_spec else None, logl_host[s])
+            if teff:
+                helios_teff_batch_host(h.ctx, p_host[s], NU_A, NU_B, logl_host[s])
+            else:
+                helios_forward_batch_host(h.ctx, p_host[s], spec_host[s] if want_spec else None, logl_host[s])
 
     def barrier():
         torch.cuda.synchronize()
@@ -229,50 +262,46 @@ def run_gpu(args):
 
     # Timing hygiene: the tables of configs[2..4] (244 MB .. 1.6 GB) exceed the 126 MB L2, so every step
     # re-reads them from HBM.  Smaller tables (configs[0], [1]) would stay L2-resident from one step to
-    # the next: then each step is timed on its own and 256 MiB are written between steps to flush L2.
+    # the next: then 256 MiB are written between steps to flush L2 and only the steps themselves are summed.
     table_bytes = wl.sigma.nbytes + wl.cia.nbytes
     flush_l2 = table_bytes < 1.5 * 126e6 and not os.environ.get("HELIOS_BENCH_NOFLUSH")
     scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush_l2 else None
 
     def timed(fn, steps, sampler=None):
+        """K steps between a barrier + synchronize on both sides.  Total = first event to last event
+        (flush time subtracted when L2 is flushed between steps); every step also has its own event
+        pair, for the median and the minimum."""
         barrier()
         if sampler:
             sampler.start()
-        if flush_l2:
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-            for e0, e1 in ev:
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for e0, e1 in ev:
+            if flush_l2:
                 scratch.zero_()
-                e0.record()
-                fn()
-                e1.record()
-            barrier()
-            ms = float(sum(e0.elapsed_time(e1) for e0, e1 in ev))
-        else:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            for _ in range(steps):
-                fn()
+            fn()
             e1.record()
-            barrier()
-            ms = e0.elapsed_time(e1)
+        barrier()
+        per_step = [e0.elapsed_time(e1) for e0, e1 in ev]
+        ms = float(sum(per_step)) if flush_l2 else ev[0][0].elapsed_time(ev[-1][1])
         clocks = sampler.stop() if sampler else None
         if world > 1:
             t = torch.tensor([ms], device=dev, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        return ms, clocks
+        return ms, clocks, per_step
 
     for _ in range(max(args.warmup, 3)):
         step_device()
     h.stats(reset=True)
     h.set_timing(True)
-    ms, clocks = timed(step_device, args.steps, ClockSampler(local) if rank == 0 else None)
+    ms, clocks, per_step = timed(step_device, args.steps, ClockSampler(local) if rank == 0 else None)
     stage = h.stage_ms()
     st = h.stats(reset=True)
     h.set_timing(False)
     for _ in range(2):
         step_host()
-    ms_host, _ = timed(step_host, args.steps)
+    ms_host, _, per_step_host = timed(step_host, args.steps)
 
     ms_step = ms / args.steps
     total_models = cfg.batch * world
@@ -283,47 +312,69 @@ def run_gpu(args):
             dist.destroy_process_group()
         return
 
-    peaks, peak_src = measured_peaks()
+    peaks, hbm_src = measured_peaks()
     fma, mufu = algorithmic_ops(cfg)
     rt_ms = stage["rt_ms"]                                    # per call, CUDA events on the ctx stream
-    ach_tflops = 2.0 * fma * B_call * cfg.n_nu / (rt_ms * 1e-3) / 1e12
+    n_sms = pk.get("n_sms", 148)
+    # peak of the binding pipe: measured FMAs per clock per SM (the better of FFMA and FFMA2) x SMs x the SM clock
+    # sampled DURING the timed region (nvidia-smi), 1 FMA = 2 flop
+    sm_mhz = (clocks or {}).get("sm_mhz") or pk["sm_clock_mhz"]
+    fma_clk = max(pk["ffma_per_clk_sm"], pk["ffma2_per_clk_sm"])
+    alu_peak = fma_clk * n_sms * 2.0 * sm_mhz * 1e6 / 1e12
+    mufu_peak = pk["mufu_per_clk_sm"] * n_sms * sm_mhz * 1e6          # results / s
+    points = B_call * cfg.n_nu
+    ach_tflops = 2.0 * fma * points / (rt_ms * 1e-3) / 1e12
+    ach_mufu = mufu * points / (rt_ms * 1e-3)
     bytes_move = must_move_bytes(cfg, B_call)
     line = {
         "metric": "forward_models_per_s", "value": value, "unit": "models/s", "n_gpus": world,
-        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+        "ms_per_step_median": float(np.median(per_step)), "ms_per_step_min": float(np.min(per_step)),
+        "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "batch": cfg.batch, "calls_per_step": n_calls,
+        "config": {"workload": wl_name, "batch": cfg.batch, "calls_per_step": n_calls,
                    "n_nu": cfg.n_nu, "n_levels": cfg.n_levels, "n_species": cfg.n_species, "n_cia": cfg.n_cia,
                    "n_angles": cfg.n_angles, "n_bins": cfg.n_bins, "spectra_written": bool(want_spec),
-                   "parallelism": f"batch-sharded x{world}, tables replicated",
-                   "l2": ("opacity table (%.0f MB) fits L2: 256 MiB written between timed steps, each step timed "
-                          "on its own" if flush_l2 else "opacity table (%.0f MB) exceeds the 126 MB L2; no flush")
+                   "parallelism": f"replicas x{world}: batch per rank, tables replicated, no collective",
+                   "l2": ("opacity table (%.0f MB) fits L2: 256 MiB written between timed steps, only the steps summed"
+                          if flush_l2 else "opacity table (%.0f MB) exceeds the 126 MB L2; no flush")
                          % (table_bytes / 1e6),
-                   "kernel": {0: "auto", 1: "direct", 2: "slab"}[args.kernel]},
+                   "kernel": {0: "auto", 1: "direct", 2: "slab", 3: "level-parallel"}[args.kernel]},
         "points_per_s": value * cfg.n_nu,
         "stage_ms_per_call": stage,
         "roofline": {"bound": "alu", "kernel": "fused interpolate+tau+RT", "achieved": ach_tflops,
-                     "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tflops / ALU_PEAK_TFLOPS,
-                     "traffic": NCU_TRAFFIC_BYTES.get(cfg.index),
-                     "peak_source": "148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (DESIGN.md)",
-                     "algorithmic_fma_per_point": fma, "algorithmic_mufu_per_point": mufu},
+                     "peak": alu_peak, "unit": "TFLOP/s", "frac": ach_tflops / alu_peak,
+                     "traffic": NCU_TRAFFIC_BYTES.get(cfg.index) if args.batch <= 0 and not teff else None,
+                     "peak_source": peak_src, "peak_fma_per_clk_sm": fma_clk, "peak_sm_mhz": sm_mhz,
+                     "algorithmic_fma_per_point": fma, "algorithmic_mufu_per_point": mufu,
+                     "mufu_frac": ach_mufu / mufu_peak, "mufu_peak_per_clk_sm": pk["mufu_per_clk_sm"],
+                     "nominal_frac": ach_tflops / (NOMINAL_FMA_PER_CLK_SM * 148 * 2 * NOMINAL_SM_MHZ * 1e6 / 1e12)},
+        "measured_peaks": pk,
         "hbm_roofline": {"must_move_bytes_per_call": bytes_move,
                          "achieved_gbs": bytes_move / (ms_step / n_calls * 1e-3) / 1e9,
                          "frac_of_8TBs": bytes_move / (ms_step / n_calls * 1e-3) / 1e9 / HBM_NOMINAL_GBS,
                          "frac_of_measured": bytes_move / (ms_step / n_calls * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                         "measured_peak_gbs": peaks["hbm_gbs"], "peak_source": peak_src},
+                         "measured_peak_gbs": peaks["hbm_gbs"], "peak_source": hbm_src,
+                         "note": "north_star's target (>= 0.6 at batch >= 256) is out of reach for this method: the path "
+                                 "is FP32/MUFU-bound there (SURVEY.md 8(d)); HBM binds only for B <= 8"},
         "e2e": {"value": e2e_value, "unit": "models/s", "h2d_bytes_per_step": cfg.batch * P * 8,
-                "d2h_bytes_per_step": cfg.batch * ((cfg.n_bins * 4 if want_spec else 0) + 8)},
+                "d2h_bytes_per_step": cfg.batch * ((cfg.n_bins * 4 if want_spec else 0) + 8),
+                "ms_per_step_median": float(np.median(per_step_host)), "ms_per_step_min": float(np.min(per_step_host))},
         "gpu_launches": st["n_launches"],
         "clocks": clocks,
     }
     if world == 1 and not args.no_cpu_baseline:
         import oracle
-        n = oracle_sample_size(wl, cfg, oracle.max_threads())
-        dt, cores = time_oracle(wl, n, min_wall_s=10.0)
+        cores = oracle.max_threads()
+        n = oracle_sample_size(wl, cfg, cores)
+        dt, _ = time_oracle(wl, n, min_wall_s=10.0, n_threads=cores)
         line["cpu_baseline"] = {"value": n / dt, "unit": "models/s", "cores": cores, "kind": "oracle",
                                 "sample": f"first {n} of {cfg.batch} models of configs[{cfg.index}], "
                                           f"all nu/levels/bins, {dt:.1f} s wall per pass, passes repeated for >= 10 s"}
+        n1 = max(1, min(n, int(round(5.0 * (n / dt) / cores))))       # about 5 s on one thread
+        dt1, _ = time_oracle(wl, n1, n_threads=1)
+        line["cpu_baseline_1thread"] = {"value": n1 / dt1, "unit": "models/s", "cores": 1, "kind": "oracle",
+                                        "sample": f"first {n1} models, one pass of {dt1:.1f} s"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -334,9 +385,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--config", type=int, default=-1, help="BASELINE.json configs index (default 3; 2 for --workload teff)")
+    ap.add_argument("--workload", default="forward", choices=["forward", "teff"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 slab")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 slab, 3 level-parallel")
     ap.add_argument("--models-per-cta", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="override the workload's batch size (sweeps only)")

@@ -49,7 +49,8 @@ enum {
 
 typedef struct helios_stats {
     unsigned long long n_clamped;      /* (model, level) pairs whose (T, p) fell outside the table and were clamped */
-    unsigned long long n_nonfinite;    /* models rejected because a parameter was NaN/Inf                          */
+    unsigned long long n_nonfinite;    /* models rejected: a parameter was NaN/Inf, or the model is unphysical
+                                          (see helios_forward_batch)                                               */
     unsigned long long n_models;       /* models evaluated since the last reset                                    */
     unsigned long long n_launches;     /* kernels launched by this context since the last reset                    */
 } helios_stats;
@@ -66,7 +67,7 @@ const char* helios_last_error(const helios_ctx* ctx);
 int  helios_set_option(helios_ctx* ctx, int key, int value);
 
 /* Opacity tables.  Copies everything to HBM as fp32,
- * nu-contiguous, rows padded to 128 B.
+ * nu-contiguous, rows padded to 256 B (64 floats, the staged kernel's tile).
  *   T_grid_K        HOST [nT]  strictly increasing, arbitrary spacing (nT >= 2)
  *   log10p_grid_bar HOST [nP]  strictly increasing, arbitrary spacing (nP >= 2)
  *   wavenumber grid nu_i = nu0_cm1 + i*dnu_cm1, i < nNu (uniform, dnu > 0)
@@ -128,35 +129,50 @@ int helios_set_observation(helios_ctx* ctx, int n_bins, const double* bin_edges_
                            const double* obs, const double* obs_err,
                            const double* inst_sigma_cm1);
 
-/* Pre-allocate workspace for batches up to max_batch (otherwise grown on demand,
- * which synchronises the device once). */
+/* Pre-allocate workspace for batches up to max_batch.  Otherwise every entry point below that
+ * takes a batch (forward_batch, loglike_batch, forward_highres, teff_batch, forward_batch_host)
+ * grows it on first use of a larger B, which synchronises the stream ONCE; after that they only
+ * enqueue. */
 int helios_reserve(helios_ctx* ctx, int max_batch);
 
-/* The hot path.  params: DEVICE, row-major [B][P] fp64, P = 2 + n_knots + n_species:
- *   log10 g (cgs), f (Eq. 9), T_knot[0..K-1] in K (bottom -> top), log10 VMR[0..S-1].
+/* The hot path.  params: DEVICE, row-major [B][n_params] fp64 with
+ *   n_params = P = 2 + N_T + n_species + n_extras  (= helios_get_n_params(); N_T = n_knots unless
+ *   helios_set_tp_elements changed it; n_extras from helios_set_extras):
+ *   log10 g (cgs), f (Eq. 9), the N_T temperature parameters (bottom -> top), log10 VMR[0..S-1],
+ *   then the extras that are switched on.
+ * n_params is the row length the CALLER built params with; a value different from
+ * helios_get_n_params() returns HELIOS_EINVAL (a buffer laid out for another parametrisation would
+ * otherwise be read with the wrong stride).
  * spectra_out: DEVICE [B][n_bins] fp32 or NULL; logl_out: DEVICE [B] fp64 or NULL.
- * A model with a non-finite parameter gets NaN spectra and logL = -inf; the
- * other models are unaffected.  Enqueues only. */
-int helios_forward_batch(helios_ctx* ctx, int B, const double* params,
+ * Rejected models get NaN spectra and logL = -inf (never NaN), the other models of the batch are
+ * unaffected, and helios_stats.n_nonfinite counts them.  A model is rejected when a parameter is
+ * NaN/Inf or when it is unphysical [paper silent; R31]: a level temperature <= 0 (possible
+ * with elements of order >= 2 or ratio parameters), sum of the VMRs > 1 (negative H2/He fill), f < 0,
+ * d <= 0, or g, 10^epsilon or a cloud parameter that overflows.  Enqueues only. */
+int helios_forward_batch(helios_ctx* ctx, int B, int n_params, const double* params,
                          float* spectra_out, double* logl_out);
-/* == helios_forward_batch(ctx, B, params, NULL, logl_out): spectra never written. */
-int helios_loglike_batch(helios_ctx* ctx, int B, const double* params, double* logl_out);
+/* == helios_forward_batch(ctx, B, n_params, params, NULL, logl_out): spectra never written. */
+int helios_loglike_batch(helios_ctx* ctx, int B, int n_params, const double* params, double* logl_out);
 /* Test hook: the flux of Eq. 9 on the native grid, before the instrument
  * profile.  flux_out: DEVICE [B][nNu] fp32.  Needs no observation. */
-int helios_forward_highres(helios_ctx* ctx, int B, const double* params, float* flux_out);
+int helios_forward_highres(helios_ctx* ctx, int B, int n_params, const double* params, float* flux_out);
 
 /* Effective temperature (Sect. 2.6): the outgoing flux F+ of Eq. 8 (without the
  * f (R/d)^2 of Eq. 9) integrated over [nu_a, nu_b] on the native grid (trapezoid, interpolated end
  * points) and converted with the Stefan-Boltzmann law.  teff_out: DEVICE [B] fp64, Kelvin.
  * Runs steps 0-4 of the hot path and one reduction kernel; needs no observation.  Enqueues only. */
-int helios_teff_batch(helios_ctx* ctx, int B, const double* params, double nu_a_cm1, double nu_b_cm1,
-                      double* teff_out);
+int helios_teff_batch(helios_ctx* ctx, int B, int n_params, const double* params, double nu_a_cm1,
+                      double nu_b_cm1, double* teff_out);
 
 /* End-to-end variant: params, spectra_out (or NULL), logl_out (or NULL) are HOST
  * buffers (pinned for full speed).  Copies params to the device, runs the hot
  * path, copies the results back and synchronises the stream before returning. */
-int helios_forward_batch_host(helios_ctx* ctx, int B, const double* params_host,
+int helios_forward_batch_host(helios_ctx* ctx, int B, int n_params, const double* params_host,
                               float* spectra_out_host, double* logl_out_host);
+
+/* The same for helios_teff_batch: HOST params [B][n_params] in, HOST teff_out [B] out. */
+int helios_teff_batch_host(helios_ctx* ctx, int B, int n_params, const double* params_host, double nu_a_cm1,
+                           double nu_b_cm1, double* teff_out_host);
 
 /* Copies the counters (synchronises the stream); reset != 0 clears them. */
 int helios_get_stats(helios_ctx* ctx, helios_stats* out, int reset);
@@ -165,6 +181,23 @@ int helios_get_stats(helios_ctx* ctx, helios_stats* out, int reset);
  * (at most the last 64), from CUDA events recorded on the context's stream.
  * HOST out: stage_ms[3], n_calls.  Synchronises the stream. */
 int helios_get_stage_ms(helios_ctx* ctx, double* stage_ms, int* n_calls);
+/* Measured arithmetic peaks of the device this context lives on (micro-benchmarks of a few hundred
+ * microseconds each: dependency-free FFMA / FFMA2 / MUFU.EX2 loops on every SM, 16 warps per scheduler).
+ * These are the denominators of the "alu" roofline bench.py reports ("the build must
+ * microbenchmark them") and the evidence for the dispatch-cost argument of DESIGN.md section 6.
+ * Runs on the context's stream and synchronises it. */
+typedef struct helios_peaks {
+    double sm_clock_mhz;        /* SM clock while the loops ran (clock64 against %globaltimer)                     */
+    double ffma_per_clk_sm;     /* FP32 FMAs per clock per SM through scalar FFMA                                   */
+    double ffma2_per_clk_sm;    /* FP32 FMAs per clock per SM through packed FFMA2 (fma.rn.f32x2)                   */
+    double mufu_per_clk_sm;     /* MUFU.EX2 results per clock per SM                                                */
+    double ffma2_cycles[3];     /* scheduler cycles one FFMA2 warp instruction occupies when its source operands
+                                   are 1 register pair + 2 scalars / 2 pairs + 1 scalar / 3 distinct pairs          */
+    double alu_extra_cycles;    /* extra scheduler cycles per LOP3 issued among FFMA2 (1.0 = no co-issue)           */
+    double fsel_extra_cycles;   /* extra scheduler cycles per FSETP + FSEL pair issued among FFMA2                  */
+    int    n_sms;
+} helios_peaks;
+int helios_measure_peaks(helios_ctx* ctx, helios_peaks* out);
 /* HOST out: the angle set in use, mu[n_angles], w[n_angles]. */
 int helios_get_angles(const helios_ctx* ctx, double* mu_out, double* w_out);
 

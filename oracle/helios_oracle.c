@@ -472,8 +472,8 @@ void oracle_cloud_dtau(int L, const double *p_bar, double tau_c, double p_top_c,
  * params [B][P], P = 2 + K + S: log10 g (cgs), f, T_knot[0..K-1] (bottom->top),
  * log10 VMR[0..S-1].   Outputs (any may be NULL): flux_hr [B][nNu] (Eq. 9,
  * before the instrument profile), spectra [B][J], logl [B].
- * obs/err may be NULL when logl is NULL.  A model with a non-finite parameter
- * gets NaN spectra and logl = -inf (R-nonfinite).
+ * obs/err may be NULL when logl is NULL.  A model with a non-finite parameter,
+ * or an unphysical one (R31, see below), gets NaN spectra and logl = -inf.
  * Returns the number of (model, level) pairs whose (T, p) was clamped.
  * ---------------------------------------------------------------------- */
 #define ORACLE_EXTRA_DISTANCE        1u   /* + d:   F = F+ f flux_const / d^2 (Eq. 9, flux_const = R_*^2)   */
@@ -543,6 +543,26 @@ long oracle_forward_ext(int S, int nT, const double *T_grid, int nP, const doubl
         } else
             oracle_temperature_profile(L, p_bar, K, T_par, p_bot_bar, p_top_bar, T);   /* O0 */
         oracle_mixing_ratios(S, log10_vmr, he_to_h2, x, &x_h2, &x_he);              /* O0 */
+
+        /* Unphysical models are rejected like non-finite ones [paper silent; R31]: a level
+         * temperature <= 0 (possible with elements of order >= 2 or ratio parameters), VMRs summing to
+         * more than 1 (negative H2/He fill), f < 0, d <= 0, or g / 10^eps / a cloud parameter overflowing. */
+        {
+            int ok = isfinite(g_cgs) && f >= 0.0 && x_h2 + x_he >= 0.0;
+            for (int l = 0; l < L; ++l) if (!(T[l] > 0.0) || !isfinite(T[l])) ok = 0;
+            if (i_d >= 0 && !(th[i_d] > 0.0)) ok = 0;
+            if (i_eps >= 0 && !isfinite(pow(10.0, th[i_eps]))) ok = 0;
+            if (i_cloud >= 0 && (!isfinite(pow(10.0, th[i_cloud])) ||
+                                 !isfinite(pow(10.0, th[i_cloud + 1]) * (1.0 + pow(10.0, th[i_cloud + 2]))))) ok = 0;
+            if (!ok) {
+                if (flux_hr) for (int k = 0; k < nNu; ++k) flux_hr[(size_t)b * nNu + k] = NAN;
+                if (spectra) for (int j = 0; j < J; ++j) spectra[(size_t)b * J + j] = NAN;
+                if (logl) logl[b] = -INFINITY;
+                if (teff) teff[b] = NAN;
+                free(p_bar); free(T); free(x);
+                continue;
+            }
+        }
 
         /* chi[l][nu], then dtau[l][nu] */
         double *chi = (double *)malloc(sizeof(double) * (size_t)L * nNu);

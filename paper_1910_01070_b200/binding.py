@@ -40,6 +40,12 @@ class helios_stats(C.Structure):
                 ("n_models", C.c_ulonglong), ("n_launches", C.c_ulonglong)]
 
 
+class helios_peaks(C.Structure):
+    _fields_ = [("sm_clock_mhz", C.c_double), ("ffma_per_clk_sm", C.c_double), ("ffma2_per_clk_sm", C.c_double),
+                ("mufu_per_clk_sm", C.c_double), ("ffma2_cycles", C.c_double * 3), ("alu_extra_cycles", C.c_double),
+                ("fsel_extra_cycles", C.c_double), ("n_sms", C.c_int)]
+
+
 _lib = None
 
 
@@ -65,23 +71,25 @@ def lib() -> C.CDLL:
                                             C.c_double, C.c_double, C.c_double]
         L.helios_set_observation.argtypes = [_vp, C.c_int, _dp, _dp, _dp, _dp]
         L.helios_reserve.argtypes = [_vp, C.c_int]
-        L.helios_forward_batch.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
-        L.helios_loglike_batch.argtypes = [_vp, C.c_int, _vp, _vp]
-        L.helios_forward_highres.argtypes = [_vp, C.c_int, _vp, _vp]
-        L.helios_forward_batch_host.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
+        L.helios_forward_batch.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp, _vp]
+        L.helios_loglike_batch.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
+        L.helios_forward_highres.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp]
+        L.helios_forward_batch_host.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp, _vp]
         L.helios_get_stats.argtypes = [_vp, C.POINTER(helios_stats), C.c_int]
         L.helios_get_angles.argtypes = [_vp, _dp, _dp]
         L.helios_get_stage_ms.argtypes = [_vp, _dp, C.POINTER(C.c_int)]
         L.helios_set_tp_elements.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
         L.helios_set_extras.argtypes = [_vp, C.c_uint]
         L.helios_get_n_params.argtypes = [_vp, C.POINTER(C.c_int)]
-        L.helios_teff_batch.argtypes = [_vp, C.c_int, _vp, C.c_double, C.c_double, _vp]
+        L.helios_teff_batch.argtypes = [_vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
+        L.helios_measure_peaks.argtypes = [_vp, C.POINTER(helios_peaks)]
+        L.helios_teff_batch_host.argtypes = [_vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
         for name in ("helios_create", "helios_set_stream", "helios_set_option", "helios_load_opacity",
                      "helios_set_atmosphere", "helios_set_observation", "helios_reserve",
                      "helios_forward_batch", "helios_loglike_batch", "helios_forward_highres",
                      "helios_forward_batch_host", "helios_get_stats", "helios_get_angles",
                      "helios_get_stage_ms", "helios_set_tp_elements", "helios_set_extras", "helios_get_n_params",
-                     "helios_teff_batch"):
+                     "helios_teff_batch", "helios_measure_peaks", "helios_teff_batch_host"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -183,39 +191,56 @@ def helios_get_n_params(ctx: int) -> int:
     return n.value
 
 
+def _rows(params):
+    """(B, P) of a 2-D parameter block; the C side checks P against the context."""
+    if params.ndim != 2:
+        raise ValueError("params must be 2-D [B][n_params]")
+    return int(params.shape[0]), int(params.shape[1])
+
+
 def helios_teff_batch(ctx: int, params, nu_a_cm1: float, nu_b_cm1: float, teff_out) -> None:
     """params: CUDA float64 [B][P]; teff_out: CUDA float64 [B]."""
-    _check(ctx, lib().helios_teff_batch(_vp(ctx), params.shape[0], _dev_ptr(params, "float64"), float(nu_a_cm1),
-                                        float(nu_b_cm1), _dev_ptr(teff_out, "float64")))
+    B, P = _rows(params)
+    _check(ctx, lib().helios_teff_batch(_vp(ctx), B, P, _dev_ptr(params, "float64"), float(nu_a_cm1),
+                                        float(nu_b_cm1), _dev_ptr(teff_out, "float64", (B,))))
 
 
 def helios_reserve(ctx: int, max_batch: int) -> None:
     _check(ctx, lib().helios_reserve(_vp(ctx), int(max_batch)))
 
 
-def _dev_ptr(t, dtype_name: str):
+def _dev_ptr(t, dtype_name: str, shape=None):
     if t is None:
         return _vp(0)
     import torch
     want = getattr(torch, dtype_name)
     if not (t.is_cuda and t.dtype == want and t.is_contiguous()):
         raise ValueError(f"expected a contiguous CUDA tensor of dtype {dtype_name}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected an output tensor of shape {tuple(shape)}, got {tuple(t.shape)}")
     return _vp(t.data_ptr())
 
 
 def helios_forward_batch(ctx: int, params, spectra_out=None, logl_out=None) -> None:
     """params: CUDA float64 [B][P]; spectra_out: CUDA float32 [B][J] or None; logl_out: CUDA float64 [B] or None."""
-    _check(ctx, lib().helios_forward_batch(_vp(ctx), params.shape[0], _dev_ptr(params, "float64"),
-                                           _dev_ptr(spectra_out, "float32"), _dev_ptr(logl_out, "float64")))
+    B, P = _rows(params)
+    if spectra_out is not None and (spectra_out.ndim != 2 or spectra_out.shape[0] != B):
+        raise ValueError("spectra_out must be [B][n_bins]")
+    _check(ctx, lib().helios_forward_batch(_vp(ctx), B, P, _dev_ptr(params, "float64"),
+                                           _dev_ptr(spectra_out, "float32"), _dev_ptr(logl_out, "float64", (B,))))
 
 
 def helios_loglike_batch(ctx: int, params, logl_out) -> None:
-    _check(ctx, lib().helios_loglike_batch(_vp(ctx), params.shape[0], _dev_ptr(params, "float64"),
-                                           _dev_ptr(logl_out, "float64")))
+    B, P = _rows(params)
+    _check(ctx, lib().helios_loglike_batch(_vp(ctx), B, P, _dev_ptr(params, "float64"),
+                                           _dev_ptr(logl_out, "float64", (B,))))
 
 
 def helios_forward_highres(ctx: int, params, flux_out) -> None:
-    _check(ctx, lib().helios_forward_highres(_vp(ctx), params.shape[0], _dev_ptr(params, "float64"),
+    B, P = _rows(params)
+    if flux_out is None or flux_out.ndim != 2 or flux_out.shape[0] != B:
+        raise ValueError("flux_out must be [B][n_nu]")
+    _check(ctx, lib().helios_forward_highres(_vp(ctx), B, P, _dev_ptr(params, "float64"),
                                              _dev_ptr(flux_out, "float32")))
 
 
@@ -223,8 +248,10 @@ def _host_ptr(a, dtype):
     if a is None:
         return _vp(0)
     if hasattr(a, "data_ptr"):           # (pinned) CPU torch tensor
-        if a.is_cuda or not a.is_contiguous():
-            raise ValueError("expected a contiguous HOST tensor")
+        import torch
+        want = {np.float64: torch.float64, np.float32: torch.float32}[dtype]
+        if a.is_cuda or not a.is_contiguous() or a.dtype != want:
+            raise ValueError(f"expected a contiguous HOST tensor of dtype {want}")
         return _vp(a.data_ptr())
     if a.dtype != dtype or not a.flags["C_CONTIGUOUS"]:
         raise ValueError(f"expected a C-contiguous numpy array of dtype {dtype}")
@@ -233,9 +260,21 @@ def _host_ptr(a, dtype):
 
 def helios_forward_batch_host(ctx: int, params_host, spectra_out_host=None, logl_out_host=None) -> None:
     """HOST buffers (numpy or pinned CPU tensors): H2D copy, hot path, D2H copy, stream sync."""
-    _check(ctx, lib().helios_forward_batch_host(_vp(ctx), params_host.shape[0], _host_ptr(params_host, np.float64),
+    B, P = _rows(params_host)
+    for out, n in ((spectra_out_host, None), (logl_out_host, 1)):
+        if out is not None and (out.shape[0] != B or (n == 1 and out.ndim != 1)):
+            raise ValueError("output buffers must have B rows")
+    _check(ctx, lib().helios_forward_batch_host(_vp(ctx), B, P, _host_ptr(params_host, np.float64),
                                                 _host_ptr(spectra_out_host, np.float32),
                                                 _host_ptr(logl_out_host, np.float64)))
+
+
+def helios_teff_batch_host(ctx: int, params_host, nu_a_cm1: float, nu_b_cm1: float, teff_out_host) -> None:
+    B, P = _rows(params_host)
+    if teff_out_host is None or teff_out_host.ndim != 1 or teff_out_host.shape[0] != B:
+        raise ValueError("teff_out_host must be [B]")
+    _check(ctx, lib().helios_teff_batch_host(_vp(ctx), B, P, _host_ptr(params_host, np.float64), float(nu_a_cm1),
+                                             float(nu_b_cm1), _host_ptr(teff_out_host, np.float64)))
 
 
 def helios_get_stats(ctx: int, reset: bool = False) -> dict:
@@ -249,6 +288,14 @@ def helios_get_stage_ms(ctx: int) -> dict:
     n = C.c_int()
     _check(ctx, lib().helios_get_stage_ms(_vp(ctx), ms, C.byref(n)))
     return {"prep_ms": ms[0], "rt_ms": ms[1], "obs_ms": ms[2], "n_calls": n.value}
+
+
+def helios_measure_peaks(ctx: int) -> dict:
+    pk = helios_peaks()
+    _check(ctx, lib().helios_measure_peaks(_vp(ctx), C.byref(pk)))
+    out = {k: getattr(pk, k) for k, _ in helios_peaks._fields_ if k != "ffma2_cycles"}
+    out["ffma2_cycles"] = list(pk.ffma2_cycles)
+    return out
 
 
 def helios_get_angles(ctx: int, n_angles: int):
@@ -297,7 +344,7 @@ class Helios:
                        he_to_h2, flux_const=1.0):
         helios_set_atmosphere(self.ctx, n_levels, p_bottom_bar, p_top_bar, n_knots, n_angles,
                               mean_mol_weight, he_to_h2, flux_const)
-        self.n_params = 2 + n_knots + self._n_species
+        self.n_params = helios_get_n_params(self.ctx)     # extras survive this call; the context knows P
 
     def set_observation(self, bin_edges, obs=None, obs_err=None, inst_sigma=None):
         helios_set_observation(self.ctx, bin_edges, obs, obs_err, inst_sigma)
@@ -362,3 +409,6 @@ class Helios:
 
     def stats(self, reset=False):
         return helios_get_stats(self.ctx, reset)
+
+    def measure_peaks(self) -> dict:
+        return helios_measure_peaks(self.ctx)

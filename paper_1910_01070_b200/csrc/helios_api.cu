@@ -14,6 +14,7 @@
 #include "../../include/helios.h"
 #include "common.cuh"
 #include "obs.cuh"
+#include "peaks.cuh"
 #include "prep.cuh"
 #include "rt_direct.cuh"
 #include "rt_slab.cuh"
@@ -200,6 +201,33 @@ static bool build_tensor_maps(helios_ctx* c) {
     }
     c->have_tmaps = true;
     return true;
+}
+
+// One micro-benchmark: exactly one resident wave (n_sms x blocks-per-SM blocks), so that the clock64() span of
+// block 0 is the time its SM needed for ALL of its resident blocks.  Returns scheduler cycles per warp instruction.
+template <int MODE>
+static int run_peak(helios_ctx* c, float* d_out, PeakTimes* d_times, double* cycles_per_instr, double* sm_ops_per_clk,
+                    double* mhz) {
+    int resident = 0;
+    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_peak<MODE>, kPeakThreads, 0));
+    if (resident < 1) return fail(c, HELIOS_ECUDA, "measure_peaks: kernel does not fit an SM");
+    if (resident > 4) resident = 4;
+    PeakTimes best{0, 0};
+    for (int rep = 0; rep < 3; ++rep) {      // the first repetition warms the clocks up; keep the fastest
+        k_peak<MODE><<<c->num_sms * resident, kPeakThreads, 0, c->stream>>>(d_out, d_times, 0.999f, 0.001f, 5u);
+        c->n_launches += 1;
+        CU_TRY(c, cudaGetLastError());
+        PeakTimes t;
+        CU_TRY(c, cudaMemcpyAsync(&t, d_times, sizeof t, cudaMemcpyDeviceToHost, c->stream));
+        CU_TRY(c, cudaStreamSynchronize(c->stream));
+        if (rep == 0 || t.cycles < best.cycles) best = t;
+    }
+    const double thread_ops = (double)kPeakIters * kPeakChains;
+    const double warps_per_scheduler = resident * (kPeakThreads / 32) / 4.0;
+    *cycles_per_instr = (double)best.cycles / (thread_ops * warps_per_scheduler);
+    *sm_ops_per_clk = thread_ops * resident * kPeakThreads / (double)best.cycles;
+    *mhz = best.ns > 0 ? 1e3 * (double)best.cycles / (double)best.ns : 0.0;
+    return HELIOS_OK;
 }
 
 extern "C" {
@@ -486,6 +514,10 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
         row_ptr[j + 1] = row_ptr[j] + (hi - lo + 1);
     }
     int* d_klo = nullptr; int* d_khi = nullptr; double* d_sig = nullptr; double* d_norm = nullptr;
+    struct Temporaries {      // freed on every return path, also the CU_TRY early returns
+        int*& a; int*& b; double*& s; double*& n;
+        ~Temporaries() { dfree(a); dfree(b); dfree(s); dfree(n); }
+    } temporaries{d_klo, d_khi, d_sig, d_norm};
     std::vector<double> sig;
     if (inst_sigma) sig.assign(inst_sigma, inst_sigma + c->nNu);
     CU_TRY(c, upload(c->d_edges, e, c->stream));
@@ -505,7 +537,6 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
     c->n_launches += 2;
     CU_TRY(c, cudaGetLastError());
     CU_TRY(c, cudaStreamSynchronize(c->stream));
-    dfree(d_klo); dfree(d_khi); dfree(d_sig); dfree(d_norm);
 
     if (obs) {
         std::vector<double> o(obs, obs + J), i2v(J);
@@ -597,6 +628,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
     pa.counters = c->d_counters;
     stamp(c, 0);
+    CU_TRY(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int) * B, c->stream));
     k_prep<<<(B * c->L + 127) / 128, 128, 0, c->stream>>>(pa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
@@ -620,7 +652,10 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     da.sigma = c->d_sigma; da.cia = c->d_cia; da.S = c->S; da.C = c->C; da.nT = c->nT; da.nP = c->nP; da.nNu = c->nNu;
     da.L = c->L; da.stride = c->stride; da.rec = c->d_rec; da.rec_floats = rf; da.model_scale = c->d_scale;
     da.model_flag = c->d_flag; da.nu0 = c->nu0; da.dnu = c->dnu; da.flux = flux; da.flux_stride = flux_stride; da.ang = c->ang;
-    const size_t smem = sizeof(float) * (size_t)c->L * rf;
+    const size_t smem = sizeof(float) * (size_t)c->L * rf;     // the direct kernel keeps one model's records in shared memory
+    if (smem > c->smem_optin)
+        return fail(c, HELIOS_EINVAL, "direct kernel: n_levels x record size (%zu B) exceeds the %zu B of shared memory a "
+                    "block may use, and the staged kernel is unavailable for this table shape", smem, c->smem_optin);
     const dim3 grid((c->nNu + kDirectThreads - 1) / kDirectThreads, B);
 #define HELIOS_DIRECT_CASE(N)                                                                               \
     case N:                                                                                                 \
@@ -639,20 +674,21 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     return HELIOS_OK;
 }
 
-static int check_ready(helios_ctx* c, int B, const double* params, bool need_obs, bool need_data) {
+static int check_ready(helios_ctx* c, int B, int P, const double* params, bool need_obs, bool need_data) {
     if (!c) return HELIOS_EINVAL;
     if (!c->have_tables || !c->have_atmo) return fail(c, HELIOS_ESTATE, "tables and atmosphere must be set first");
     if (need_obs && !c->have_obs) return fail(c, HELIOS_ESTATE, "observation grid not set (helios_set_observation)");
     if (need_data && !c->have_data) return fail(c, HELIOS_ESTATE, "logL requested but the observation has no data");
     if (B < 1 || B > 65535) return fail(c, HELIOS_EINVAL, "batch %d out of range (1..65535)", B);
     if (!params) return fail(c, HELIOS_EINVAL, "params is NULL");
-    if ((size_t)c->L * std::max(direct_rec_floats(c->S, c->C), 4) * sizeof(float) > 200 * 1024)
-        return fail(c, HELIOS_EINVAL, "n_levels x record size exceeds shared memory");
+    if (P != n_params(c))
+        return fail(c, HELIOS_EINVAL, "n_params %d does not match this context's parameter vector (2 + %d temperature "
+                    "parameters + %d species + %d extras = %d)", P, c->NT, c->S, c->n_extra, n_params(c));
     return HELIOS_OK;
 }
 
-int helios_forward_highres(helios_ctx* c, int B, const double* params, float* flux_out) {
-    int rc = check_ready(c, B, params, false, false);
+int helios_forward_highres(helios_ctx* c, int B, int P, const double* params, float* flux_out) {
+    int rc = check_ready(c, B, P, params, false, false);
     if (rc) return rc;
     if (!flux_out) return fail(c, HELIOS_EINVAL, "flux_out is NULL");
     CU_TRY(c, cudaSetDevice(c->device));
@@ -663,8 +699,8 @@ int helios_forward_highres(helios_ctx* c, int B, const double* params, float* fl
     return rc;
 }
 
-int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spectra_out, double* logl_out) {
-    int rc = check_ready(c, B, params, true, logl_out != nullptr);
+int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, float* spectra_out, double* logl_out) {
+    int rc = check_ready(c, B, P, params, true, logl_out != nullptr);
     if (rc) return rc;
     if (!spectra_out && !logl_out) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
     CU_TRY(c, cudaSetDevice(c->device));
@@ -685,9 +721,9 @@ int helios_forward_batch(helios_ctx* c, int B, const double* params, float* spec
     return HELIOS_OK;
 }
 
-int helios_loglike_batch(helios_ctx* c, int B, const double* params, double* logl_out) {
+int helios_loglike_batch(helios_ctx* c, int B, int P, const double* params, double* logl_out) {
     if (c && !logl_out) return fail(c, HELIOS_EINVAL, "logl_out is NULL");
-    return helios_forward_batch(c, B, params, nullptr, logl_out);
+    return helios_forward_batch(c, B, P, params, nullptr, logl_out);
 }
 
 int helios_set_tp_elements(helios_ctx* c, int n_elements, int order, int ratio_form) {
@@ -720,8 +756,8 @@ int helios_get_n_params(const helios_ctx* c, int* out) {
     return HELIOS_OK;
 }
 
-int helios_teff_batch(helios_ctx* c, int B, const double* params, double nu_a, double nu_b, double* teff_out) {
-    int rc = check_ready(c, B, params, false, false);
+int helios_teff_batch(helios_ctx* c, int B, int P, const double* params, double nu_a, double nu_b, double* teff_out) {
+    int rc = check_ready(c, B, P, params, false, false);
     if (rc) return rc;
     if (!teff_out) return fail(c, HELIOS_EINVAL, "teff_out is NULL");
     const double nu_first = c->nu0, nu_last = c->nu0 + c->dnu * (c->nNu - 1);
@@ -740,21 +776,35 @@ int helios_teff_batch(helios_ctx* c, int B, const double* params, double nu_a, d
     return HELIOS_OK;
 }
 
-int helios_forward_batch_host(helios_ctx* c, int B, const double* params_host, float* spectra_host, double* logl_host) {
-    int rc = check_ready(c, B, params_host, true, logl_host != nullptr);
+int helios_forward_batch_host(helios_ctx* c, int B, int P_in, const double* params_host, float* spectra_host, double* logl_host) {
+    int rc = check_ready(c, B, P_in, params_host, true, logl_host != nullptr);
     if (rc) return rc;
     if (!spectra_host && !logl_host) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
     CU_TRY(c, cudaSetDevice(c->device));
     if ((rc = helios_reserve(c, B))) return rc;
     const size_t P = n_params(c);
     CU_TRY(c, cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * P, cudaMemcpyHostToDevice, c->stream));
-    rc = helios_forward_batch(c, B, c->d_params_stage, spectra_host ? c->d_spectra_stage : nullptr,
+    rc = helios_forward_batch(c, B, P_in, c->d_params_stage, spectra_host ? c->d_spectra_stage : nullptr,
                               logl_host ? c->d_logl_stage : nullptr);
     if (rc) return rc;
     if (spectra_host)
         CU_TRY(c, cudaMemcpyAsync(spectra_host, c->d_spectra_stage, sizeof(float) * (size_t)B * c->J, cudaMemcpyDeviceToHost, c->stream));
     if (logl_host)
         CU_TRY(c, cudaMemcpyAsync(logl_host, c->d_logl_stage, sizeof(double) * B, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return HELIOS_OK;
+}
+
+int helios_teff_batch_host(helios_ctx* c, int B, int P_in, const double* params_host, double nu_a, double nu_b,
+                           double* teff_host) {
+    int rc = check_ready(c, B, P_in, params_host, false, false);
+    if (rc) return rc;
+    if (!teff_host) return fail(c, HELIOS_EINVAL, "teff_out is NULL");
+    CU_TRY(c, cudaSetDevice(c->device));
+    if ((rc = helios_reserve(c, B))) return rc;
+    CU_TRY(c, cudaMemcpyAsync(c->d_params_stage, params_host, sizeof(double) * B * (size_t)P_in, cudaMemcpyHostToDevice, c->stream));
+    if ((rc = helios_teff_batch(c, B, P_in, c->d_params_stage, nu_a, nu_b, c->d_logl_stage))) return rc;
+    CU_TRY(c, cudaMemcpyAsync(teff_host, c->d_logl_stage, sizeof(double) * B, cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     return HELIOS_OK;
 }
@@ -774,6 +824,34 @@ int helios_get_stage_ms(helios_ctx* c, double* stage_ms, int* n_calls) {
     }
     stage_ms[0] = n ? acc[0] / n : 0; stage_ms[1] = n ? acc[1] / n : 0; stage_ms[2] = n_obs ? acc[2] / n_obs : 0;
     *n_calls = n;
+    return HELIOS_OK;
+}
+
+int helios_measure_peaks(helios_ctx* c, helios_peaks* out) {
+    if (!c || !out) return HELIOS_EINVAL;
+    CU_TRY(c, cudaSetDevice(c->device));
+    float* d_out = nullptr; PeakTimes* d_times = nullptr;
+    CU_TRY(c, cudaMalloc(&d_out, sizeof(float) * (size_t)c->num_sms * 4 * kPeakThreads));
+    if (cudaMalloc(&d_times, sizeof(PeakTimes)) != cudaSuccess) { cudaFree(d_out); return fail(c, HELIOS_ENOMEM, "measure_peaks: out of memory"); }
+    double cyc[kPeakModes] = {}, ops[kPeakModes] = {}, mhz[kPeakModes] = {};
+    int rc = HELIOS_OK;
+    if (!rc) rc = run_peak<kPeakFfma>(c, d_out, d_times, &cyc[0], &ops[0], &mhz[0]);
+    if (!rc) rc = run_peak<kPeakFfma2Scalar>(c, d_out, d_times, &cyc[1], &ops[1], &mhz[1]);
+    if (!rc) rc = run_peak<kPeakFfma2TwoPairs>(c, d_out, d_times, &cyc[2], &ops[2], &mhz[2]);
+    if (!rc) rc = run_peak<kPeakFfma2ThreePairs>(c, d_out, d_times, &cyc[3], &ops[3], &mhz[3]);
+    if (!rc) rc = run_peak<kPeakMufuEx2>(c, d_out, d_times, &cyc[4], &ops[4], &mhz[4]);
+    if (!rc) rc = run_peak<kPeakFfma2PlusAlu>(c, d_out, d_times, &cyc[5], &ops[5], &mhz[5]);
+    if (!rc) rc = run_peak<kPeakFfma2PlusFsel>(c, d_out, d_times, &cyc[6], &ops[6], &mhz[6]);
+    cudaFree(d_out); cudaFree(d_times);
+    if (rc) return rc;
+    out->n_sms = c->num_sms;
+    out->sm_clock_mhz = mhz[1];
+    out->ffma_per_clk_sm = ops[0];
+    out->ffma2_per_clk_sm = 2.0 * ops[1];
+    out->mufu_per_clk_sm = ops[4];
+    for (int i = 0; i < 3; ++i) out->ffma2_cycles[i] = cyc[1 + i];
+    out->alu_extra_cycles = cyc[5] - cyc[1];       // modes 5 and 6 count one FFMA2 + one extra op (pair) per "instruction"
+    out->fsel_extra_cycles = cyc[6] - cyc[1];
     return HELIOS_OK;
 }
 

@@ -31,8 +31,8 @@ struct PrepArgs {
     float* model_x;           // DEVICE [B][x_floats]  staged kernel: x_s 2^32, x_H2 x_c
     int x_floats;
     float* model_scale;       // DEVICE [B]  f * flux_const * 2 pi
-    int*   model_flag;        // DEVICE [B]  1 = non-finite parameter
-    unsigned long long* counters;  // [0] clamped pairs, [1] non-finite models
+    int*   model_flag;        // DEVICE [B]  1 = rejected model (zeroed before the launch, raised by any thread of the model)
+    unsigned long long* counters;  // [0] clamped pairs, [1] rejected models
 };
 
 constexpr int kMaxTpNodes = 5;    // order <= 4
@@ -61,26 +61,41 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     bool finite = true;
     for (int i = 0; i < a.P; ++i) finite = finite && isfinite(th[i]);
     float* rec = a.rec + ((size_t)b * a.L + l) * a.rec_floats;
-    if (l == 0) {
-        a.model_flag[b] = finite ? 0 : 1;
-        double scale = a.unit_scale ? 1.0 : th[1] * a.flux_const;
-        int ie = 2 + a.NT + a.S;
-        if (a.extras & 1u) { if (!a.unit_scale) scale /= th[ie] * th[ie]; ++ie; }     // distance, Eq. 9
-        a.model_addvar[b] = (a.extras & 2u) ? pow(10.0, th[ie]) : 0.0;                 // error inflation, Eq. 22
-        a.model_scale[b] = finite ? (float)(scale * 2.0 * kPi) : 0.0f;
-        if (!finite) atomicAdd(&a.counters[1], 1ULL);
+    const int i_extra = 2 + a.NT + a.S;
+    const double* tpar = th + 2;
+    const double* lvmr = th + 2 + a.NT;
+    // Rejected models (helios.h, R31): a non-finite parameter, or an unphysical model -- a level
+    // temperature <= 0, VMRs summing to more than 1, f < 0, d <= 0, or a derived quantity that overflows.
+    // model_flag is zeroed before the launch; any thread of the model may raise it.
+    double T = 0.0, T_up = 0.0, xsum = 0.0;
+    bool ok = finite;
+    if (finite) {
+        T = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l], a.lvl_lw + (size_t)l * kMaxTpNodes);
+        if (l + 1 < a.L)
+            T_up = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l + 1], a.lvl_lw + (size_t)(l + 1) * kMaxTpNodes);
+        for (int s = 0; s < a.S; ++s) xsum += pow(10.0, lvmr[s]);
+        ok = T > 0.0 && isfinite(T) && (l + 1 >= a.L || (T_up > 0.0 && isfinite(T_up))) && xsum <= 1.0 &&
+             isfinite(pow(10.0, th[0])) && th[1] >= 0.0;
+        int ie = i_extra;
+        if (a.extras & 1u) { ok = ok && th[ie] > 0.0; ++ie; }
+        if (a.extras & 2u) { ok = ok && isfinite(pow(10.0, th[ie])); ++ie; }
+        if (a.extras & 4u) ok = ok && isfinite(pow(10.0, th[ie])) && isfinite(pow(10.0, th[ie + 1]) * (1.0 + pow(10.0, th[ie + 2])));
     }
-    if (!finite) {
+    if (!ok && atomicOr(&a.model_flag[b], 1) == 0) atomicAdd(&a.counters[1], 1ULL);
+    if (l == 0) {
+        double scale = a.unit_scale ? 1.0 : th[1] * a.flux_const;
+        int ie = i_extra;
+        if (a.extras & 1u) { if (!a.unit_scale) scale /= th[ie] * th[ie]; ++ie; }     // distance, Eq. 9
+        a.model_addvar[b] = (ok && (a.extras & 2u)) ? pow(10.0, th[ie]) : 0.0;         // error inflation, Eq. 22
+        a.model_scale[b] = ok ? (float)(scale * 2.0 * kPi) : 0.0f;
+    }
+    if (!ok) {
         for (int i = 0; i < a.rec_floats; ++i) rec[i] = 0.0f;
         if (l == 0 && a.slab_layout) for (int i = 0; i < a.x_floats; ++i) a.model_x[(size_t)b * a.x_floats + i] = 0.0f;
         return;
     }
 
     const double g = pow(10.0, th[0]);
-    const double* tpar = th + 2;
-    const double* lvmr = th + 2 + a.NT;
-
-    const double T = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l], a.lvl_lw + (size_t)l * kMaxTpNodes);
     const double p = a.lvl_p_bar[l];
 
     // temperature cell: largest iT with T_grid[iT] <= T, clamped to [0, nT-2]
@@ -95,8 +110,6 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     const double u = a.lvl_u[l];
 
     const double n = p * kBarCgs / (kBoltzmann * T);     // cm^-3
-    double xsum = 0.0;
-    for (int s = 0; s < a.S; ++s) xsum += pow(10.0, lvmr[s]);
     const double x_bg = 1.0 - xsum;
     const double x_h2 = x_bg / (1.0 + a.he_to_h2);
     const double x_he = x_bg * a.he_to_h2 / (1.0 + a.he_to_h2);
@@ -141,8 +154,6 @@ __global__ void __launch_bounds__(128) k_prep(PrepArgs a) {
     }
     double hdz = 0.0, dtc = 0.0;
     if (l + 1 < a.L) {
-        double T_up = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l + 1],
-                                        a.lvl_lw + (size_t)(l + 1) * kMaxTpNodes);
         double dz = kBoltzmann * 0.5 * (T + T_up) / (a.mmw * kAtomicMass * g) * a.lvl_lnratio[l];
         hdz = 0.5 * dz;
         if (a.extras & 4u) {

@@ -65,6 +65,71 @@ def _relerr(a, ref):
     return float(np.max(np.abs(a / ref - 1.0)))
 
 
+H_PLANCK, C_LIGHT, K_B = 6.62607015e-27, 2.99792458e10, 1.380649e-16
+
+
+def _check_flux_bounds(cfg, params, flux, n_t=None, rtol=2e-6):
+    """SURVEY.md section 4 invariant, on every model: each intensity is a convex combination of level
+    sources, so pi f B_nu(T_min) <= F <= pi f B_nu(T_max) with the extremes of the model's own profile
+    (piecewise linear in log p: extremes at the nodes).  Planck is evaluated here, in fp64."""
+    n_t = cfg.n_knots if n_t is None else n_t
+    nu = cfg.nu0 + cfg.dnu * np.arange(cfg.n_nu)
+    c1, c2 = 2 * H_PLANCK * C_LIGHT ** 2, H_PLANCK * C_LIGHT / K_B
+    for b in range(params.shape[0]):
+        T = params[b, 2:2 + n_t]
+        f = params[b, 1] * cfg.flux_const
+        lo = np.pi * f * c1 * nu ** 3 / np.expm1(c2 * nu / T.min())
+        hi = np.pi * f * c1 * nu ** 3 / np.expm1(c2 * nu / T.max())
+        assert np.all(flux[b] >= lo * (1 - rtol)) and np.all(flux[b] <= hi * (1 + rtol)), b
+
+
+class _Obs:
+    def __init__(self, obs, obs_err):
+        self.obs, self.obs_err = np.asarray(obs, np.float64), np.asarray(obs_err, np.float64)
+
+
+def _logl_from_spectrum(wl, spec):
+    """Eq. 19 in fp64 (scipy's normal log-density) from a binned spectrum [B][J]."""
+    from scipy.stats import norm
+    return norm.logpdf(wl.obs[None, :], loc=spec, scale=wl.obs_err[None, :]).sum(axis=1)
+
+
+def _check_logl(wl, logl, ref, spec_gpu=None, tag=None):
+    """logL against the oracle.  north_star's 1e-3 ABSOLUTE bound is asserted wherever it is attainable
+    (reduced chi-square of order 1: the near-truth tests).  Far from the truth |logL| reaches 1e5..1e6 and
+    a binned-flux error e_j (allowed: 1e-4 M_j) moves logL by up to sum_j (|D_j - M_j| e_j + e_j^2/2)/sigma_j^2:
+    that propagated bound is asserted on every model, and -- tighter -- that the chi-square reduction
+    itself is exact: logL equals Eq. 19 evaluated in fp64 on the GPU's own binned spectrum."""
+    M = ref["spectra"]
+    e = TOL_FLUX * np.abs(M)
+    bound = ((np.abs(wl.obs[None, :] - M) * e + 0.5 * e * e) / wl.obs_err[None, :] ** 2).sum(axis=1)
+    d = np.abs(logl - ref["logl"])
+    assert np.all(d <= bound + TOL_LOGL_ABS), (float(d.max()), float(bound.min()))
+    if spec_gpu is not None:
+        own = _logl_from_spectrum(wl, spec_gpu)
+        assert np.max(np.abs(logl - own) / np.maximum(1.0, np.abs(own))) <= 1e-9
+    _record(tag, max_abs_dlogl=float(d.max()), max_rel_dlogl=float(np.max(d / np.maximum(1.0, np.abs(ref["logl"])))),
+            max_abs_logl=float(np.abs(ref["logl"]).max()), n_models=int(len(d)))
+    return float(d.max())
+
+
+def _record(tag, **kv):
+    """Measured maxima go to gpurun_out/parity_summary.json (scratch; the numbers quoted in DESIGN.md
+    'logL tolerance' come from it)."""
+    if tag is None:
+        return
+    import json, os
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    try:
+        os.makedirs(out, exist_ok=True)
+        path = os.path.join(out, "parity_summary.json")
+        data = json.load(open(path)) if os.path.exists(path) else {}
+        data.setdefault(tag, {}).update(kv)
+        json.dump(data, open(path, "w"), indent=1, sort_keys=True)
+    except OSError:
+        pass
+
+
 @pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
 def test_config0_tiny(torch_cuda, oracle, wl0, kernel):
     ref = oracle.forward_workload(wl0, want_flux=True)
@@ -81,9 +146,8 @@ def test_config1_medium_all_models(torch_cuda, oracle, wl1, kernel):
     spec, logl, flux, st = _run(torch_cuda, wl1, wl1.params, kernel)
     assert _relerr(flux, ref["flux_hr"]) <= TOL_FLUX
     assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
-    # far from the truth |logL| ~ 1e5..1e6: the absolute bound is not meaningful there
-    # (DESIGN.md); the relative one is.
-    assert np.max(np.abs(logl - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
+    _check_logl(wl1, logl, ref, spec, tag=f"configs[1] all 64 models, kernel {kernel}")
+    _check_flux_bounds(wl1.cfg, wl1.params, flux)
     assert st["n_clamped"] == ref["n_clamped"] * 2
 
 
@@ -95,23 +159,24 @@ def test_logl_near_truth_absolute_tolerance(torch_cuda, oracle, wl1, wl2, kernel
     ref = oracle.forward_workload(wl, params=params)
     spec, logl, _, _ = _run(torch_cuda, wl, params, kernel, highres=False)
     assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
-    red_chi2 = -2.0 * (ref["logl"] - ref["logl"].max()) / wl.cfg.n_bins
-    assert np.all(red_chi2 < 50.0)                           # the subset really is near the truth
+    red_chi2 = ((wl.obs[None, :] - ref["spectra"]) ** 2 / wl.obs_err[None, :] ** 2).sum(axis=1) / wl.cfg.n_bins
+    assert np.all(red_chi2 < 5.0)                            # the subset really is near the truth
     assert np.max(np.abs(logl - ref["logl"])) <= TOL_LOGL_ABS
+    _record(f"configs[{cfg_index}] near truth, kernel {kernel}", max_abs_dlogl=float(np.max(np.abs(logl - ref["logl"]))),
+            max_reduced_chi2=float(red_chi2.max()), n_models=12)
 
 
 def test_config2_full_batch_sampled_models(torch_cuda, oracle, wl2):
     """configs[2] at its full size (B = 256) in the launch configuration bench.py times
-    (kernel = auto); the oracle recomputes a seeded sample of 16 models."""
+    (kernel = auto); the oracle recomputes ALL 256 models."""
     spec, logl, flux, st = _run(torch_cuda, wl2, wl2.params, kernel=0)
-    rng = np.random.default_rng(2)
-    pick = np.sort(rng.choice(wl2.cfg.batch, 16, replace=False))
-    ref = oracle.forward_workload(wl2, params=wl2.params[pick], want_flux=True)
-    assert _relerr(flux[pick], ref["flux_hr"]) <= TOL_FLUX
-    assert _relerr(spec[pick], ref["spectra"]) <= TOL_FLUX
-    assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
-    # properties that hold for every model at any size
+    ref = oracle.forward_workload(wl2, want_flux=True)
+    assert _relerr(flux, ref["flux_hr"]) <= TOL_FLUX
+    assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
+    _check_logl(wl2, logl, ref, spec, tag="configs[2] all 256 models")
     assert np.isfinite(spec).all() and np.isfinite(logl).all() and (flux > 0).all()
+    _check_flux_bounds(wl2.cfg, wl2.params, flux)
+    assert st["n_clamped"] == ref["n_clamped"] * 2
 
 
 def test_config3_full_batch_sampled_models(torch_cuda, oracle, wl3):
@@ -119,12 +184,16 @@ def test_config3_full_batch_sampled_models(torch_cuda, oracle, wl3):
     tables) in the launch configuration bench.py times; the oracle recomputes a seeded sample."""
     spec, logl, flux, st = _run(torch_cuda, wl3, wl3.params, kernel=0)
     rng = np.random.default_rng(3)
-    pick = np.sort(rng.choice(wl3.cfg.batch, 6, replace=False))
+    pick = np.sort(rng.choice(wl3.cfg.batch, 64, replace=False))
     ref = oracle.forward_workload(wl3, params=wl3.params[pick], want_flux=True)
     assert _relerr(flux[pick], ref["flux_hr"]) <= TOL_FLUX
     assert _relerr(spec[pick], ref["spectra"]) <= TOL_FLUX
-    assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
+    _check_logl(wl3, logl[pick], ref, spec[pick], tag="configs[3] 64 of 1024 models")
+    # properties that hold for every one of the 1024 models
     assert np.isfinite(spec).all() and np.isfinite(logl).all() and (flux > 0).all()
+    own = _logl_from_spectrum(wl3, spec)
+    assert np.max(np.abs(logl - own) / np.maximum(1.0, np.abs(own))) <= 1e-9
+    _check_flux_bounds(wl3.cfg, wl3.params, flux)
 
 
 def test_config4_streamed_loglike_only(torch_cuda, oracle, wl3):
@@ -144,14 +213,14 @@ def test_config4_streamed_loglike_only(torch_cuda, oracle, wl3):
     B = 4096 // cfg4.n_calls
     for c in range(cfg4.n_calls):
         h.loglike_batch(p[c * B:(c + 1) * B], out[c * B:(c + 1) * B])
-    pick = np.sort(np.random.default_rng(4).choice(4096, 4, replace=False))
-    _, full = h.forward_batch(p[torch.as_tensor(pick, device="cuda:0")].contiguous())
+    pick = np.sort(np.random.default_rng(4).choice(4096, 64, replace=False))
+    spec_full, full = h.forward_batch(p[torch.as_tensor(pick, device="cuda:0")].contiguous())
     torch.cuda.synchronize()
     logl = out.cpu().numpy()
     assert np.isfinite(logl).all()
     assert np.array_equal(full.cpu().numpy(), logl[pick])
     ref = oracle.forward_workload(wl3, params=params[pick])
-    assert np.max(np.abs(logl[pick] - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4
+    _check_logl(wl3, logl[pick], ref, spec_full.cpu().numpy().astype(np.float64), tag="configs[4] 64 of 4096 models")
     h.close()
 
 
@@ -160,7 +229,11 @@ def test_logl_near_truth_config3(torch_cuda, oracle, wl3):
     ref = oracle.forward_workload(wl3, params=params)
     spec, logl, _, _ = _run(torch_cuda, wl3, params, 0, highres=False)
     assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
+    red_chi2 = ((wl3.obs[None, :] - ref["spectra"]) ** 2 / wl3.obs_err[None, :] ** 2).sum(axis=1) / wl3.cfg.n_bins
+    assert np.all(red_chi2 < 5.0)
     assert np.max(np.abs(logl - ref["logl"])) <= TOL_LOGL_ABS
+    _record("configs[3] near truth", max_abs_dlogl=float(np.max(np.abs(logl - ref["logl"]))),
+            max_reduced_chi2=float(red_chi2.max()), n_models=4)
 
 
 @pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
@@ -225,7 +298,7 @@ def test_ragged_sizes_and_edge_cases(torch_cuda, oracle, kernel):
         assert np.isnan(spec[3]).all() and np.isnan(flux[3]).all() and logl[3] == -np.inf
         assert _relerr(flux[ok], ref["flux_hr"][ok]) <= TOL_FLUX, (S, C, L, A, K)
         assert _relerr(spec[ok], ref["spectra"][ok]) <= TOL_FLUX, (S, C, L, A, K)
-        assert np.max(np.abs(logl[ok] - ref["logl"][ok]) / np.maximum(1.0, np.abs(ref["logl"][ok]))) <= 1e-4
+        _check_logl(_Obs(obs, err), logl[ok], {"spectra": ref["spectra"][ok], "logl": ref["logl"][ok]}, spec[ok])
         assert st["n_clamped"] == 2 * ref["n_clamped"] and st["n_nonfinite"] == 2
 
 
@@ -352,5 +425,60 @@ def test_random_shapes_staged_kernel(torch_cuda, oracle, seed):
     shape = dict(S=S, C=C, nT=nT, nP=nP, nNu=nNu, L=L, A=A, K=K, B=B)
     assert _relerr(flux.cpu().numpy().astype(np.float64), ref["flux_hr"]) <= TOL_FLUX, shape
     assert _relerr(spec.cpu().numpy().astype(np.float64), ref["spectra"]) <= TOL_FLUX, shape
-    assert np.max(np.abs(logl.cpu().numpy() - ref["logl"]) / np.maximum(1.0, np.abs(ref["logl"]))) <= 1e-4, shape
+    _check_logl(_Obs(obs, err), logl.cpu().numpy(), ref, spec.cpu().numpy().astype(np.float64))
     assert st["n_clamped"] == 2 * ref["n_clamped"], shape
+
+
+def test_n_params_is_checked(torch_cuda, wl1):
+    """A parameter block laid out for another parametrisation (wrong row length) is refused with
+    HELIOS_EINVAL by every entry point instead of being read with the wrong stride."""
+    import paper_1910_01070_b200 as pkg
+    torch = torch_cuda
+    h = pkg.Helios(0)
+    h.setup_workload(wl1)
+    good = torch.as_tensor(wl1.params[:4], device="cuda:0")
+    assert good.shape[1] == h.n_params == pkg.helios_get_n_params(h.ctx)
+    bad = torch.cat([good, torch.zeros((4, 1), dtype=torch.float64, device="cuda:0")], dim=1).contiguous()
+    for call in (lambda p: h.forward_batch(p), lambda p: h.loglike_batch(p), lambda p: h.forward_highres(p),
+                 lambda p: h.teff_batch(p, 4000.0, 12000.0),
+                 lambda p: h.forward_batch_host(p.cpu().pin_memory(), None, torch.empty(4, dtype=torch.float64).pin_memory())):
+        with pytest.raises(pkg.HeliosError) as ei:
+            call(bad)
+        assert ei.value.code == pkg.HELIOS_EINVAL
+    h.set_extras(pkg.HELIOS_EXTRA_DISTANCE)
+    h.set_atmosphere(wl1.cfg.n_levels, 300.0, 1e-3, wl1.cfg.n_knots, wl1.cfg.n_angles, 2.3, 0.17, 1.0)
+    assert h.n_params == good.shape[1] + 1          # the extras survive set_atmosphere; the wrapper follows the context
+    with pytest.raises(pkg.HeliosError):
+        h.forward_batch(good)
+    with pytest.raises(ValueError):
+        h.forward_batch(good[0])                    # 1-D
+    with pytest.raises(ValueError):
+        h.forward_batch_host(torch.as_tensor(wl1.params[:4], dtype=torch.float32).pin_memory(), None,
+                             torch.empty(4, dtype=torch.float64).pin_memory())       # fp32 host tensor
+    h.close()
+
+
+@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+def test_unphysical_models_are_rejected(torch_cuda, oracle, wl1, kernel):
+    """Finite but unphysical parameter vectors (R31) give logL = -inf (never NaN) and NaN
+    spectra, are counted, and leave their neighbours bit-identical; the oracle applies the same rule."""
+    import paper_1910_01070_b200 as pkg
+    torch = torch_cuda
+    cfg = wl1.cfg
+    K, S = cfg.n_knots, cfg.n_species
+    base = wl1.params[:8].copy()
+    params = base.copy()
+    params[1, 2 + K:2 + K + S] = -0.1          # VMRs sum to 3.2 > 1: negative H2/He fill
+    params[3, 1] = -0.5                         # f < 0
+    params[5, 0] = 400.0                        # g = 10^400 overflows
+    params[6, 2 + K - 1] = -50.0                # top temperature node below zero
+    ref = oracle.forward_workload(wl1, params=params, want_flux=True)
+    bad, good = [1, 3, 5, 6], [0, 2, 4, 7]
+    assert np.all(ref["logl"][bad] == -np.inf) and np.isnan(ref["spectra"][bad]).all()
+    spec, logl, flux, st = _run(torch, wl1, params, kernel)
+    assert np.all(logl[bad] == -np.inf) and np.isnan(spec[bad]).all() and np.isnan(flux[bad]).all()
+    assert st["n_nonfinite"] == 2 * len(bad)
+    spec0, logl0, flux0, _ = _run(torch, wl1, base, kernel)
+    assert np.array_equal(spec[good], spec0[good]) and np.array_equal(logl[good], logl0[good])
+    assert np.array_equal(flux[good], flux0[good])
+    assert _relerr(spec[good], ref["spectra"][good]) <= TOL_FLUX

@@ -522,6 +522,34 @@ def test_nonfinite_parameters(oracle):
     assert np.array_equal(r["spectra"][0], r["spectra"][2]) and np.isfinite(r["logl"][[0, 2]]).all()
 
 
+def test_unphysical_parameters_are_rejected(oracle):
+    # DESIGN.md R31 [paper silent]: finite but unphysical vectors are rejected like non-finite ones
+    # (logL = -inf, NaN spectra) instead of producing NaN or finite garbage for the sampler.
+    wl = W.make_workload(0)
+    good = wl.params[0]
+    cases = {"vmr_sum_gt_1": (4, 0.2), "negative_f": (1, -1.0), "g_overflow": (0, 400.0), "negative_T": (3, -10.0)}
+    params = np.tile(good, (len(cases) + 1, 1))
+    for i, (col, val) in enumerate(cases.values()):
+        params[i + 1, col] = val
+    obs = np.full(wl.cfg.n_bins, 1e5)
+    err = np.full(wl.cfg.n_bins, 2e3)
+    r = oracle.forward_workload(wl, params=params, obs=obs, obs_err=err, want_flux=True)
+    assert np.isfinite(r["logl"][0]) and np.isfinite(r["spectra"][0]).all()
+    for i, name in enumerate(cases):
+        assert r["logl"][i + 1] == -np.inf, name
+        assert np.isnan(r["spectra"][i + 1]).all() and np.isnan(r["flux_hr"][i + 1]).all(), name
+    # f = 0 and VMRs summing to exactly <= 1 are legal
+    edge = np.tile(good, (2, 1))
+    edge[0, 1] = 0.0
+    edge[1, 4] = math.log10(0.999)
+    r = oracle.forward_workload(wl, params=edge, obs=obs, obs_err=err)
+    assert np.isfinite(r["logl"]).all() and np.all(r["spectra"][0] == 0.0)
+    # extras: d <= 0
+    p = np.concatenate([good, [0.0]])[None, :]
+    r = oracle.forward_workload(wl, params=p, obs=obs, obs_err=err, extras=1)
+    assert r["logl"][0] == -np.inf
+
+
 def test_clamp_count(oracle):
     wl = W.make_workload(0)
     params = wl.params.copy()
