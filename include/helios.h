@@ -195,6 +195,8 @@ typedef struct helios_peaks {
                                    are 1 register pair + 2 scalars / 2 pairs + 1 scalar / 3 distinct pairs          */
     double alu_extra_cycles;    /* extra scheduler cycles per LOP3 issued among FFMA2 (1.0 = no co-issue)           */
     double fsel_extra_cycles;   /* extra scheduler cycles per FSETP + FSEL pair issued among FFMA2                  */
+    double ffma_3reg_cycles;    /* scheduler cycles of a scalar FFMA with three distinct register operands          */
+    double mufu_extra_cycles;   /* extra scheduler cycles per MUFU.EX2 issued among FFMA2 (8 FFMA2 : 8 MUFU)        */
     int    n_sms;
 } helios_peaks;
 int helios_measure_peaks(helios_ctx* ctx, helios_peaks* out);

@@ -43,7 +43,8 @@ class helios_stats(C.Structure):
 class helios_peaks(C.Structure):
     _fields_ = [("sm_clock_mhz", C.c_double), ("ffma_per_clk_sm", C.c_double), ("ffma2_per_clk_sm", C.c_double),
                 ("mufu_per_clk_sm", C.c_double), ("ffma2_cycles", C.c_double * 3), ("alu_extra_cycles", C.c_double),
-                ("fsel_extra_cycles", C.c_double), ("n_sms", C.c_int)]
+                ("fsel_extra_cycles", C.c_double), ("ffma_3reg_cycles", C.c_double), ("mufu_extra_cycles", C.c_double),
+                ("n_sms", C.c_int)]
 
 
 _lib = None

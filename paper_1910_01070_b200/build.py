@@ -8,7 +8,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-LIB_PATH = os.path.join(HERE, "libhelios_b200.so")
+# HELIOS_B200_LIB: path of an already built libhelios_b200.so to load instead of the in-tree one
+LIB_PATH = os.environ.get("HELIOS_B200_LIB") or os.path.join(HERE, "libhelios_b200.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -28,6 +29,8 @@ def sources():
 
 
 def is_stale() -> bool:
+    if os.environ.get("HELIOS_B200_LIB"):
+        return False
     if not os.path.exists(LIB_PATH):
         return True
     t = os.path.getmtime(LIB_PATH)
@@ -35,18 +38,21 @@ def is_stale() -> bool:
     return any(os.path.getmtime(s) > t for s in deps)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    if not force and not is_stale():
+def build_library(force: bool = False, verbose: bool = False, defines=(), out: str = None) -> str:
+    """nvcc -> LIB_PATH (or `out`); `defines` are extra -D macros (kernel experiments)."""
+    out = out or LIB_PATH
+    if not force and out == LIB_PATH and not is_stale():
         return LIB_PATH
-    tmp = LIB_PATH + f".tmp{os.getpid()}"
+    tmp = out + f".tmp{os.getpid()}"
     cmd = [_nvcc()] + [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += [f"-D{d}" for d in defines]
     cmd += ["-I", INCLUDE, "-o", tmp, os.path.join(CSRC, "helios_api.cu")]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
     if verbose:
         print(res.stderr)
-    os.replace(tmp, LIB_PATH)
-    return LIB_PATH
+    os.replace(tmp, out)
+    return out

@@ -40,7 +40,8 @@ __host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S +
 // Per-(model, level) record, kSlabRecFloats floats:
 //   0..3  n 2^-32 {(1-t)(1-u), (1-t)u, t(1-u), t u}   weights of G at (iT,ip), (iT,ip+1), (iT+1,ip), (iT+1,ip+1)
 //   4..5  am^2 {(1-t), t}                               weights of the CIA mix at iT, iT+1
-//   6..7  planck_a high / low      8  hdz      9  iT (int bits)      10  dtau_cloud of the layer above      11  unused
+//   6..7  planck_a high / low      8  hdz of the layer BELOW the level (levels l-1, l; 0 at level 0)      9  iT (int bits)
+//   10  dtau_cloud of the layer below      11  unused
 // Per-model vector, slab_x_floats(S, C) floats: x_s 2^32 (S values), then x_H2 x_c (C values).
 constexpr int kSlabRecFloats = 12;
 constexpr float kSlabXScale = 4294967296.0f;   // 2^32: keeps x_s sigma_s far above the fp32 denormal range

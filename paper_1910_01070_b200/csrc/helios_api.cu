@@ -203,30 +203,32 @@ static bool build_tensor_maps(helios_ctx* c) {
     return true;
 }
 
-// One micro-benchmark: exactly one resident wave (n_sms x blocks-per-SM blocks), so that the clock64() span of
-// block 0 is the time its SM needed for ALL of its resident blocks.  Returns scheduler cycles per warp instruction.
+// One micro-benchmark: one block of 1024 threads per SM, timed with CUDA events on the context's stream (the
+// launch overhead is < 1 % of the 0.5 ms a kernel takes); the SM clock during the run is block 0's
+// clock64() / %globaltimer ratio.  Returns scheduler cycles per warp instruction and operations per clock per SM.
 template <int MODE>
-static int run_peak(helios_ctx* c, float* d_out, PeakTimes* d_times, double* cycles_per_instr, double* sm_ops_per_clk,
-                    double* mhz) {
-    int resident = 0;
-    CU_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_peak<MODE>, kPeakThreads, 0));
-    if (resident < 1) return fail(c, HELIOS_ECUDA, "measure_peaks: kernel does not fit an SM");
-    if (resident > 4) resident = 4;
-    PeakTimes best{0, 0};
+static int run_peak(helios_ctx* c, float* d_out, PeakTimes* d_times, cudaEvent_t e0, cudaEvent_t e1,
+                    double* cycles_per_instr, double* sm_ops_per_clk, double* mhz) {
+    double best_ms = 0.0, best_mhz = 0.0;
     for (int rep = 0; rep < 3; ++rep) {      // the first repetition warms the clocks up; keep the fastest
-        k_peak<MODE><<<c->num_sms * resident, kPeakThreads, 0, c->stream>>>(d_out, d_times, 0.999f, 0.001f, 5u);
+        CU_TRY(c, cudaEventRecord(e0, c->stream));
+        k_peak<MODE><<<c->num_sms, kPeakThreads, 0, c->stream>>>(d_out, d_times, 0.999f, 0.001f, 5u);
+        CU_TRY(c, cudaEventRecord(e1, c->stream));
         c->n_launches += 1;
         CU_TRY(c, cudaGetLastError());
         PeakTimes t;
         CU_TRY(c, cudaMemcpyAsync(&t, d_times, sizeof t, cudaMemcpyDeviceToHost, c->stream));
         CU_TRY(c, cudaStreamSynchronize(c->stream));
-        if (rep == 0 || t.cycles < best.cycles) best = t;
+        float ms = 0.0f;
+        CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep == 0 || ms < best_ms) { best_ms = ms; best_mhz = t.ns > 0 ? 1e3 * (double)t.cycles / (double)t.ns : 0.0; }
     }
+    const double cycles = best_ms * 1e-3 * best_mhz * 1e6;
     const double thread_ops = (double)kPeakIters * kPeakChains;
-    const double warps_per_scheduler = resident * (kPeakThreads / 32) / 4.0;
-    *cycles_per_instr = (double)best.cycles / (thread_ops * warps_per_scheduler);
-    *sm_ops_per_clk = thread_ops * resident * kPeakThreads / (double)best.cycles;
-    *mhz = best.ns > 0 ? 1e3 * (double)best.cycles / (double)best.ns : 0.0;
+    const double warps_per_scheduler = (kPeakThreads / 32) / 4.0;
+    *cycles_per_instr = cycles / (thread_ops * warps_per_scheduler);
+    *sm_ops_per_clk = thread_ops * kPeakThreads / cycles;
+    *mhz = best_mhz;
     return HELIOS_OK;
 }
 
@@ -287,8 +289,8 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value < 0 || value > 2) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1 or 2");
             c->opt_kernel = value; return HELIOS_OK;
         case HELIOS_OPT_MODELS_PER_CTA:
-            if (value != 0 && value != 8 && value != 16 && value != 24)
-                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16 or 24");
+            if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24)
+                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16, 20 or 24");
             c->opt_models_per_cta = value; return HELIOS_OK;
         case HELIOS_OPT_TIMING:
             c->opt_timing = value ? 1 : 0; c->timed_calls = 0;
@@ -566,7 +568,6 @@ static SlabPlan plan_slab(const helios_ctx* c, int B) {
     int nw = c->opt_models_per_cta;
     if (nw == 0) {
         if (B < 16) nw = 8;
-        else if (c->A > 4) nw = 16;
         else {      // padded model slots, weighted by the measured per-model efficiency of the two variants
             const double cost24 = (double)((B + 23) / 24 * 24), cost16 = (double)((B + 15) / 16 * 16) / 0.92;
             nw = cost24 <= cost16 ? 24 : 16;
@@ -628,8 +629,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
     pa.counters = c->d_counters;
     stamp(c, 0);
-    CU_TRY(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int) * B, c->stream));
-    k_prep<<<(B * c->L + 127) / 128, 128, 0, c->stream>>>(pa);
+    k_prep<<<B, kPrepThreads, 0, c->stream>>>(pa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
     stamp(c, 1);
@@ -831,18 +831,24 @@ int helios_measure_peaks(helios_ctx* c, helios_peaks* out) {
     if (!c || !out) return HELIOS_EINVAL;
     CU_TRY(c, cudaSetDevice(c->device));
     float* d_out = nullptr; PeakTimes* d_times = nullptr;
-    CU_TRY(c, cudaMalloc(&d_out, sizeof(float) * (size_t)c->num_sms * 4 * kPeakThreads));
+    CU_TRY(c, cudaMalloc(&d_out, sizeof(float) * (size_t)c->num_sms * kPeakThreads));
     if (cudaMalloc(&d_times, sizeof(PeakTimes)) != cudaSuccess) { cudaFree(d_out); return fail(c, HELIOS_ENOMEM, "measure_peaks: out of memory"); }
     double cyc[kPeakModes] = {}, ops[kPeakModes] = {}, mhz[kPeakModes] = {};
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
     int rc = HELIOS_OK;
-    if (!rc) rc = run_peak<kPeakFfma>(c, d_out, d_times, &cyc[0], &ops[0], &mhz[0]);
-    if (!rc) rc = run_peak<kPeakFfma2Scalar>(c, d_out, d_times, &cyc[1], &ops[1], &mhz[1]);
-    if (!rc) rc = run_peak<kPeakFfma2TwoPairs>(c, d_out, d_times, &cyc[2], &ops[2], &mhz[2]);
-    if (!rc) rc = run_peak<kPeakFfma2ThreePairs>(c, d_out, d_times, &cyc[3], &ops[3], &mhz[3]);
-    if (!rc) rc = run_peak<kPeakMufuEx2>(c, d_out, d_times, &cyc[4], &ops[4], &mhz[4]);
-    if (!rc) rc = run_peak<kPeakFfma2PlusAlu>(c, d_out, d_times, &cyc[5], &ops[5], &mhz[5]);
-    if (!rc) rc = run_peak<kPeakFfma2PlusFsel>(c, d_out, d_times, &cyc[6], &ops[6], &mhz[6]);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = fail(c, HELIOS_ECUDA, "measure_peaks: cudaEventCreate failed");
+    if (!rc) rc = run_peak<kPeakFfma>(c, d_out, d_times, e0, e1, &cyc[0], &ops[0], &mhz[0]);
+    if (!rc) rc = run_peak<kPeakFfma2Scalar>(c, d_out, d_times, e0, e1, &cyc[1], &ops[1], &mhz[1]);
+    if (!rc) rc = run_peak<kPeakFfma2TwoPairs>(c, d_out, d_times, e0, e1, &cyc[2], &ops[2], &mhz[2]);
+    if (!rc) rc = run_peak<kPeakFfma2ThreePairs>(c, d_out, d_times, e0, e1, &cyc[3], &ops[3], &mhz[3]);
+    if (!rc) rc = run_peak<kPeakMufuEx2>(c, d_out, d_times, e0, e1, &cyc[4], &ops[4], &mhz[4]);
+    if (!rc) rc = run_peak<kPeakFfma2PlusAlu>(c, d_out, d_times, e0, e1, &cyc[5], &ops[5], &mhz[5]);
+    if (!rc) rc = run_peak<kPeakFfma2PlusFsel>(c, d_out, d_times, e0, e1, &cyc[6], &ops[6], &mhz[6]);
+    if (!rc) rc = run_peak<kPeakFfma3Reg>(c, d_out, d_times, e0, e1, &cyc[7], &ops[7], &mhz[7]);
+    if (!rc) rc = run_peak<kPeakFfma2PlusMufu>(c, d_out, d_times, e0, e1, &cyc[8], &ops[8], &mhz[8]);
     cudaFree(d_out); cudaFree(d_times);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
     if (rc) return rc;
     out->n_sms = c->num_sms;
     out->sm_clock_mhz = mhz[1];
@@ -852,6 +858,8 @@ int helios_measure_peaks(helios_ctx* c, helios_peaks* out) {
     for (int i = 0; i < 3; ++i) out->ffma2_cycles[i] = cyc[1 + i];
     out->alu_extra_cycles = cyc[5] - cyc[1];       // modes 5 and 6 count one FFMA2 + one extra op (pair) per "instruction"
     out->fsel_extra_cycles = cyc[6] - cyc[1];
+    out->ffma_3reg_cycles = cyc[7];
+    out->mufu_extra_cycles = cyc[8] - cyc[1];
     return HELIOS_OK;
 }
 

@@ -24,6 +24,8 @@
 //   large dtau/mu_k:  H <- e H + (1 - e) q,            e = 2^(-dtau log2e / mu_k), q = dS / dtau
 //   small dtau/mu_k:  H <- H + P_k(dtau) (dS - dtau H), P_k(dtau) = phi(dtau/mu_k) / mu_k
 // (common.cuh, R10); Planck and optical depth as in rt_direct.cuh.
+// The thin/thick branch is taken per wavenumber, but a warp whose lanes all agree (for all angles, or for the
+// small-mu / large-mu half of them) evaluates only that branch (LayerLimits).
 #pragma once
 #include <cuda.h>
 
@@ -155,6 +157,64 @@ __device__ __forceinline__ void all_angles(float2 (&H)[A], float2 dtau, float2 n
                                            std::integer_sequence<int, K...>) {
     (angle_step<A, K>(H[K], dtau, ndtau, q, dS), ...);
 }
+// The same update when the branch is known for the whole warp (bitwise the value angle_step selects).
+template <int A, int K>
+__device__ __forceinline__ void angle_step_thick(float2& H, float2 ndtau, float2 q) {
+    constexpr float c_exp = (float)(kLog2e / kGLmu[A - 1][K]);
+    const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+    H = __ffma2_rn(e, H, __ffma2_rn(neg2(e), q, q));
+}
+template <int A, int K>
+__device__ __forceinline__ void angle_step_thin(float2& H, float2 dtau, float2 ndtau, float2 dS) {
+    constexpr double mu = kGLmu[A - 1][K];
+    constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                    p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+    float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+    P = __ffma2_rn(dtau, P, bc2(p2));
+    P = __ffma2_rn(dtau, P, bc2(p1));
+    P = __ffma2_rn(dtau, P, bc2(p0));
+    H = __ffma2_rn(P, __ffma2_rn(ndtau, H, dS), H);
+}
+template <int A, int... K>
+__device__ __forceinline__ void all_angles_thick(float2 (&H)[A], float2 ndtau, float2 q, std::integer_sequence<int, K...>) {
+    (angle_step_thick<A, K>(H[K], ndtau, q), ...);
+}
+template <int A, int... K>
+__device__ __forceinline__ void all_angles_thin(float2 (&H)[A], float2 dtau, float2 ndtau, float2 dS,
+                                                std::integer_sequence<int, K...>) {
+    (angle_step_thin<A, K>(H[K], dtau, ndtau, dS), ...);
+}
+// General (per-lane) step in the "w form": H <- H + w (q - H), w = 1 - e^{-D} from ex2 (thick lanes) or from the
+// polynomial, w = dtau P_k(dtau) (thin lanes); dtau is clamped to >= 1e-20 by the caller so that q = dS / dtau is finite
+// (below that the layer is transparent to every digit either way).
+template <int A, int K>
+__device__ __forceinline__ void angle_step_w(float2& H, float2 dtau, float2 ndtau, float2 q) {
+    constexpr double mu = kGLmu[A - 1][K];
+    constexpr float c_exp = (float)(kLog2e / mu), thr = (float)(0.25 * mu);
+    constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                    p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+    const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+    const float2 wk = __fadd2_rn(bc2(1.0f), neg2(make_float2(ex2_approx(arg.x), ex2_approx(arg.y))));
+    float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+    P = __ffma2_rn(dtau, P, bc2(p2));
+    P = __ffma2_rn(dtau, P, bc2(p1));
+    P = __ffma2_rn(dtau, P, bc2(p0));
+    const float2 wn = __fmul2_rn(dtau, P);
+    const float2 w = make_float2(dtau.x < thr ? wn.x : wk.x, dtau.y < thr ? wn.y : wk.y);
+    H = __ffma2_rn(w, __fadd2_rn(q, neg2(H)), H);
+}
+// angles K0 .. K1-1 with one kind of step: 0 general, 1 thick only, 2 thin only, 3 general in the w form
+template <int A, int K0, int K1, int MODE>
+__device__ __forceinline__ void angle_range(float2 (&H)[A], float2 dtau, float2 ndtau, float2 q, float2 dS) {
+    if constexpr (K0 < K1) {
+        if constexpr (MODE == 0) angle_step<A, K0>(H[K0], dtau, ndtau, q, dS);
+        if constexpr (MODE == 1) angle_step_thick<A, K0>(H[K0], ndtau, q);
+        if constexpr (MODE == 2) angle_step_thin<A, K0>(H[K0], dtau, ndtau, dS);
+        if constexpr (MODE == 3) angle_step_w<A, K0>(H[K0], dtau, ndtau, q);
+        angle_range<A, K0 + 1, K1, MODE>(H, dtau, ndtau, q, dS);
+    }
+}
 template <int A, int K>
 __device__ __forceinline__ void flux_term(float2& acc, float2 H) {
     constexpr float wH = (float)(kGLw[A - 1][K] * kGLmu[A - 1][K] * kGLmu[A - 1][K]);
@@ -166,6 +226,16 @@ __device__ __forceinline__ float2 flux_sum(const float2 (&H)[A], float2 S_top, s
     (flux_term<A, K>(acc, H[K]), ...);
     return acc;
 }
+
+// Warp-uniform shortcuts of a layer:
+//   all-thin   every lane has dtau < 0.25 mu_0        -> only the polynomial branch, for every angle
+//   all-thick  every lane has dtau >= 0.25 mu_{A-1}   -> only the ex2 branch, for every angle
+// dtau >= 0, so the order of the floats is the order of their bit patterns (REDUX works on integers).
+template <int A>
+struct LayerLimits {
+    static constexpr unsigned all_thick = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][A - 1]));
+    static constexpr unsigned all_thin = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][0]));
+};
 
 // shared memory: [ring][S*nT*64] planes | [C*nT*64] CIA | [NW][x_floats] | mbarriers
 __host__ __device__ inline size_t slab_plane_floats(int S, int nT) { return (size_t)S * nT * kSlabTile; }
@@ -235,7 +305,8 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
     constexpr uint32_t kRowB = kSlabTile * sizeof(float);   // bytes per table row in a plane
     const uint32_t spB = a.nT * kRowB;        // bytes between species in a plane
-    const float4* rp = reinterpret_cast<const float4*>(a.rec + (size_t)b * a.L * kSlabRecFloats);
+    const float* rec_b = a.rec + (size_t)b * a.L * kSlabRecFloats;
+    const float4* rp = reinterpret_cast<const float4*>(rec_b);
     const uint32_t planes_a = smem_u32(planes) + lane * 8;   // shared-memory byte addresses of this lane's pair
     const uint32_t cia_a = smem_u32(cia_s) + lane * 8;
     const uint32_t xw_a = smem_u32(xw), xc_a = xw_a + a.S * 4;
@@ -245,7 +316,6 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 #pragma unroll
     for (int k = 0; k < A; ++k) H[k] = make_float2(0.0f, 0.0f);
     float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
-    float hdz_prev = 0.0f, dtc_prev = 0.0f;
     float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
     int released = 0, cur_iT = -2, prev_lo = -1;
 
@@ -295,7 +365,6 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             chi = __ffma2_rn(bc2(r0.w), G11, chi);
             chi = __ffma2_rn(bc2(r1.x), Gc0, chi);
             chi = __ffma2_rn(bc2(r1.y), Gc1, chi);
-            // S_l = B_nu(T_l) = c1 nu^3 E / (1 - E), E = 2^(-a nu), a nu carried as a two-float product
             const float2 ah = bc2(r1.z);
             const float2 pr = __fmul2_rn(ah, nu);
             float2 rr = __ffma2_rn(ah, nu, neg2(pr));
@@ -306,13 +375,41 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             const float2 om = __fadd2_rn(bc2(1.0f), neg2(E));
             const float2 Sl = __fmul2_rn(c1nu3, __fmul2_rn(E, make_float2(rcp_approx(om.x), rcp_approx(om.y))));
             if (l > 0) {
-                const float2 dtau = __ffma2_rn(__fadd2_rn(chi, chi_prev), bc2(hdz_prev), bc2(dtc_prev));
+                // dtau of the layer below this level: trapezoid of chi times the hydrostatic thickness, plus the grey cloud
+                const float2 dtau = __ffma2_rn(__fadd2_rn(chi, chi_prev), bc2(r2.x), bc2(r2.z));
                 const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
-                const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
                 const float2 ndtau = neg2(dtau);
-                all_angles<A>(H, dtau, ndtau, q, dS, std::make_integer_sequence<int, A>{});
+                const unsigned d_lo = __reduce_min_sync(0xffffffffu, __float_as_uint(fminf(dtau.x, dtau.y)));
+                const unsigned d_hi = __reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(dtau.x, dtau.y)));
+                if (d_hi < LayerLimits<A>::all_thin) {
+                    all_angles_thin<A>(H, dtau, ndtau, dS, std::make_integer_sequence<int, A>{});
+                } else {
+                    const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
+                    if (d_lo >= LayerLimits<A>::all_thick) {
+                        all_angles_thick<A>(H, ndtau, q, std::make_integer_sequence<int, A>{});
+                    } else {
+                        constexpr int GM = 3;
+                        const float2 dtc = make_float2(fmaxf(dtau.x, 1e-20f), fmaxf(dtau.y, 1e-20f));
+                        const float2 ndtc = neg2(dtc);
+                        const float2 qc = __fmul2_rn(dS, make_float2(rcp_approx(dtc.x), rcp_approx(dtc.y)));
+                        // many angles: the small-mu half is often thick for every lane while the large-mu half is
+                        // still mixed, or the large-mu half thin while the small-mu half is mixed (measured: pays for A >= 6)
+                        constexpr int AH = A >= 6 ? A / 2 : 0;
+                        constexpr unsigned kLowThick = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][AH > 0 ? AH - 1 : 0]));
+                        constexpr unsigned kHighThin = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][AH]));
+                        if (AH > 0 && d_lo >= kLowThick) {
+                            angle_range<A, 0, AH, 1>(H, dtau, ndtau, q, dS);
+                            angle_range<A, AH, A, GM>(H, dtc, ndtc, qc, dS);
+                        } else if (AH > 0 && d_hi < kHighThin) {
+                            angle_range<A, 0, AH, GM>(H, dtc, ndtc, qc, dS);
+                            angle_range<A, AH, A, 2>(H, dtau, ndtau, q, dS);
+                        } else {
+                            angle_range<A, 0, A, GM>(H, dtc, ndtc, qc, dS);
+                        }
+                    }
+                }
             }
-            chi_prev = chi; S_prev = Sl; hdz_prev = r2.x; dtc_prev = r2.z;
+            chi_prev = chi; S_prev = Sl;
         }
         if (a.S > 0 && seg + 1 < a.n_seg) {
             // slots holding loads older than the next segment's are free for the producer
@@ -353,7 +450,7 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
     SlabPlan p;
     if (A < 1 || A > kMaxAngles || nT > 256) return p;
     const int nw = want_nw > 0 ? want_nw : 16;
-    if (nw != 8 && nw != 16 && nw != 24) return p;
+    if (nw != 8 && nw != 16 && nw != 20 && nw != 24) return p;
     const int target_ctas = nw == 8 ? 3 : 1;
     const size_t plane = sizeof(float) * slab_plane_floats(S, nT);
     const size_t fixed = slab_fixed_bytes(C, nT, nw, slab_x_floats(S, C));
@@ -396,6 +493,7 @@ inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& t
     switch (p.NW) {
         case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p.smem, stream);
         case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p.smem, stream);
+        case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p.smem, stream);
         case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p.smem, stream);
         default: return cudaErrorInvalidValue;
     }
