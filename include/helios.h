@@ -42,8 +42,9 @@ enum {
 #define HELIOS_PTRS_ON_DEVICE 1u   /* helios_load_opacity: sigma[s] / cia[c] are DEVICE pointers */
 
 /* helios_set_option keys */
-#define HELIOS_OPT_KERNEL      1   /* 0 = auto (staged whenever the table planes fit shared memory), 1 = direct (4 taps from
-                                      global memory; fallback), 2 = staged TMA kernel (error if unavailable) */
+#define HELIOS_OPT_KERNEL      1   /* 0 = auto (level-parallel for a handful of models, else staged whenever the table planes fit
+                                      shared memory, else direct), 1 = direct (4 taps from global memory; fallback),
+                                      2 = staged TMA kernel, 3 = level-parallel kernel (2, 3: error if unavailable) */
 #define HELIOS_OPT_MODELS_PER_CTA 2/* staged kernel: models (= compute warps) per CTA: 8, 16, 24 or 0 = auto */
 #define HELIOS_OPT_TIMING      3   /* 1 = bracket every stage of the next calls with CUDA events on the context's stream */
 

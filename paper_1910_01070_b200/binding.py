@@ -21,7 +21,7 @@ HELIOS_PTRS_ON_DEVICE = 1
 HELIOS_OPT_KERNEL = 1
 HELIOS_OPT_MODELS_PER_CTA = 2
 HELIOS_OPT_TIMING = 3
-KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB = 0, 1, 2
+KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB, KERNEL_LEVEL_PARALLEL = 0, 1, 2, 3
 HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD = 1, 2, 4
 
 _dp = C.POINTER(C.c_double)

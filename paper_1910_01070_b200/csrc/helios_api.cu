@@ -18,6 +18,7 @@
 #include "prep.cuh"
 #include "rt_direct.cuh"
 #include "rt_slab.cuh"
+#include "rt_seg.cuh"
 
 using namespace helios;
 
@@ -53,7 +54,8 @@ struct helios_ctx {
     std::vector<int> lvl_ip;
     // staged kernel: plane schedule (segments of constant pressure cell) and TMA views of the tables
     int n_seg = 0, n_loads = 0;
-    int* d_seg_lbegin = nullptr; int* d_seg_hi = nullptr; int* d_seg_lo = nullptr; int* d_load_ip = nullptr;
+    SlabSeg* d_seg = nullptr;           // [kSlabMaxRing][n_seg]: the schedule resolved for every ring depth
+    int* d_load_ip = nullptr;
     bool have_tmaps = false;
     CUtensorMap tm_sigma{}, tm_cia{};
     size_t smem_optin = 0, smem_sm = 0;
@@ -122,7 +124,7 @@ static void free_all(helios_ctx* c) {
     dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid);
     dfree(c->d_lvl_p); dfree(c->d_lvl_elem); dfree(c->d_lvl_lw); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
     dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
-    dfree(c->d_seg_lbegin); dfree(c->d_seg_hi); dfree(c->d_seg_lo); dfree(c->d_load_ip);
+    dfree(c->d_seg); dfree(c->d_load_ip);
     dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_var); dfree(c->d_addvar); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x); dfree(c->d_counters);
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
@@ -286,7 +288,7 @@ int helios_set_option(helios_ctx* c, int key, int value) {
     if (!c) return HELIOS_EINVAL;
     switch (key) {
         case HELIOS_OPT_KERNEL:
-            if (value < 0 || value > 2) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1 or 2");
+            if (value < 0 || value > 3) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1, 2 or 3");
             c->opt_kernel = value; return HELIOS_OK;
         case HELIOS_OPT_MODELS_PER_CTA:
             if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24)
@@ -433,9 +435,27 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
         }
         seg_lbegin.push_back(L);
         c->n_seg = (int)seg_hi.size(); c->n_loads = (int)load_ip.size();
-        CU_TRY(c, upload(c->d_seg_lbegin, seg_lbegin, c->stream));
-        CU_TRY(c, upload(c->d_seg_hi, seg_hi, c->stream));
-        CU_TRY(c, upload(c->d_seg_lo, seg_lo, c->stream));
+        // slot / mbarrier parity of every load and the slots each segment frees, for every ring depth NB:
+        // load e lives in slot e % NB during its use number e / NB; a segment frees the loads older than the next one's
+        std::vector<SlabSeg> seg((size_t)kSlabMaxRing * c->n_seg);
+        for (int nb = 1; nb <= kSlabMaxRing; ++nb) {
+            int released = 0;
+            for (int k = 0; k < c->n_seg; ++k) {
+                SlabSeg& g = seg[(size_t)(nb - 1) * c->n_seg + k];
+                g.l_begin = seg_lbegin[k]; g.l_end = seg_lbegin[k + 1];
+                g.hi = (seg_hi[k] % nb) | (((seg_hi[k] / nb) & 1) << 8);
+                g.lo = (seg_lo[k] % nb) | (((seg_lo[k] / nb) & 1) << 8);
+                g.shifted = (k > 0 && seg_hi[k] == seg_lo[k - 1]) ? 1 : 0;
+                g.rel_slot = 0; g.rel_count = 0; g.pad = 0;
+                if (k + 1 < c->n_seg) {
+                    const int next_first = std::min(seg_hi[k + 1], seg_lo[k + 1]);
+                    g.rel_slot = released % nb;
+                    g.rel_count = std::max(0, next_first - released);
+                    released = std::max(released, next_first);
+                }
+            }
+        }
+        CU_TRY(c, upload(c->d_seg, seg, c->stream));
         CU_TRY(c, upload(c->d_load_ip, load_ip, c->stream));
     }
 
@@ -560,6 +580,9 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
     return HELIOS_OK;
 }
 
+constexpr int kSegAutoMaxBatch = 4;       // measured crossover with the staged kernel (profiles/r02_batch_sweep.md)
+constexpr int kObsSmallBatchCtas = 592;     // 4 CTAs of 8 warps per SM on 148 SMs
+
 static SlabPlan plan_slab(const helios_ctx* c, int B) {
     SlabPlan none;
     if (c->opt_kernel == 1 || !c->have_tmaps) return none;
@@ -595,7 +618,7 @@ int helios_reserve(helios_ctx* c, int B) {
     CU_TRY(c, cudaMalloc(&c->d_flag, sizeof(int) * B));
     CU_TRY(c, cudaMalloc(&c->d_model_x, sizeof(float) * (size_t)B * slab_x_floats(c->S, c->C)));
     {
-        const int n_chunks = ((c->J > 0 ? c->J : 1) + kObsBinsPerCta - 1) / kObsBinsPerCta;
+        const int n_chunks = ((c->J > 0 ? c->J : 1) + 7) / 8;       // the finer of the two chunkings of k_obs_apply
         CU_TRY(c, cudaMalloc(&c->d_obs_partial, sizeof(double) * (size_t)B * n_chunks));
         CU_TRY(c, cudaMalloc(&c->d_obs_arrived, sizeof(unsigned) * B));
         CU_TRY(c, cudaMemsetAsync(c->d_obs_arrived, 0, sizeof(unsigned) * B, c->stream));
@@ -617,7 +640,12 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     const SlabPlan plan = plan_slab(c, B);
     if (c->opt_kernel == 2 && !plan.ok)
         return fail(c, HELIOS_EINVAL, "staged kernel requested but unavailable for this table shape (shared memory / TMA)");
-    const int slab = plan.ok ? 1 : 0;
+    // level-parallel kernel: small batches (measured crossover, profiles/r02_batch_sweep.md), or on request
+    const SegPlan seg = (c->opt_kernel == 3 || (c->opt_kernel == 0 && B <= kSegAutoMaxBatch))
+                            ? seg_plan(c->L, c->A, c->S, c->C, slab_x_floats(c->S, c->C), c->smem_optin) : SegPlan{};
+    if (c->opt_kernel == 3 && !seg.ok)
+        return fail(c, HELIOS_EINVAL, "level-parallel kernel requested but unavailable for %d levels", c->L);
+    const int slab = (plan.ok || seg.ok) ? 1 : 0;      // both use the staged-kernel records
     const int rf = slab ? kSlabRecFloats : direct_rec_floats(c->S, c->C);
     PrepArgs pa{};
     pa.params = params; pa.B = B; pa.P = n_params(c); pa.K = c->K; pa.S = c->S; pa.C = c->C; pa.L = c->L;
@@ -634,13 +662,25 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     CU_TRY(c, cudaGetLastError());
     stamp(c, 1);
 
+    if (seg.ok) {
+        SegArgs ga{};
+        ga.sigma = c->d_sigma; ga.cia = c->d_cia; ga.stride = c->stride; ga.S = c->S; ga.C = c->C; ga.nT = c->nT; ga.nP = c->nP;
+        ga.nNu = c->nNu; ga.L = c->L; ga.B = B; ga.rec = c->d_rec; ga.model_x = c->d_model_x; ga.x_floats = pa.x_floats;
+        ga.model_scale = c->d_scale; ga.model_flag = c->d_flag; ga.lvl_ip = c->d_lvl_ip; ga.nu0 = c->nu0; ga.dnu = c->dnu;
+        ga.flux = flux; ga.flux_stride = flux_stride; ga.n_chunks = seg.n_chunks; ga.chunk_len = seg.chunk_len;
+        cudaError_t e = launch_rt_seg(c->A, ga, seg.smem, c->stream);
+        if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "level-parallel kernel launch failed: %s", cudaGetErrorString(e));
+        c->n_launches += 1;
+        stamp(c, 2);
+        return HELIOS_OK;
+    }
     if (slab) {
         SlabArgs sa{};
         sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nNu = c->nNu; sa.L = c->L; sa.B = B;
         sa.rec = c->d_rec; sa.model_x = c->d_model_x; sa.x_floats = pa.x_floats;
         sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu;
         sa.flux = flux; sa.flux_stride = flux_stride;
-        sa.seg_lbegin = c->d_seg_lbegin; sa.seg_hi = c->d_seg_hi; sa.seg_lo = c->d_seg_lo; sa.load_ip = c->d_load_ip;
+        sa.seg = c->d_seg + (size_t)(plan.ring - 1) * c->n_seg; sa.load_ip = c->d_load_ip;
         sa.n_seg = c->n_seg; sa.n_loads = c->n_loads; sa.ring = plan.ring; sa.ang = c->ang;
         cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->stream);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "staged kernel launch failed: %s", cudaGetErrorString(e));
@@ -713,7 +753,12 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     if (c->extras & HELIOS_EXTRA_ERROR_INFLATION) { oa.var = c->d_var; oa.addvar = c->d_addvar; }
     oa.logl_const = c->logl_const; oa.spectra = spectra_out; oa.logl = logl_out;
     oa.partial = c->d_obs_partial; oa.arrived = c->d_obs_arrived;
-    k_obs_apply<<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa);
+    // one bin per warp while 64-bin CTAs would leave SMs idle (the choice depends on B only through this threshold;
+    // kObsSmallBatchCtas is fixed, so a given (B, J) always takes the same variant)
+    if ((long long)B * ((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta) < kObsSmallBatchCtas)
+        k_obs_apply<1><<<dim3((c->J + 7) / 8, B), kObsThreads, 0, c->stream>>>(oa);
+    else
+        k_obs_apply<8><<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa);
     c->n_launches += 1;
     CU_TRY(c, cudaGetLastError());
     stamp(c, 3);

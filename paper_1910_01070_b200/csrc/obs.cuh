@@ -92,24 +92,27 @@ struct ObsApplyArgs {
 };
 
 constexpr int kObsThreads = 256;
-constexpr int kObsBinsPerCta = 64;   // 8 warps x 8 bins
+constexpr int kObsBinsPerCta = 64;   // 8 warps x 8 bins (large batches); 8 warps x 1 bin for a handful of models
 
 // One CTA per (model, chunk of 64 bins): B * J / 64 CTAs keep every SM busy (one CTA per model
 // left 14 warps per SM waiting on dependent L2 loads).  Each warp owns 8 bins: lanes stride the
 // band of W, a shuffle tree finishes M_j, lane 0 adds the chi-square term in fp64.  The chunk
 // sums go to `partial`; the CTA that finishes a model last (atomic ticket) adds them in chunk
 // order, so logL is bitwise reproducible, and only logL is written when spectra == nullptr.
+// With a handful of models B * J / 64 CTAs do not fill the GPU and the 8 bins of a warp are 8 chains of dependent
+// loads one after the other: kPerWarp = 1 gives every bin its own warp (8 bins per CTA).
+template <int kPerWarp>
 __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
     __shared__ double warp_sum[kObsThreads / 32];
     __shared__ unsigned ticket;
     const int b = blockIdx.y, chunk = blockIdx.x, n_chunks = gridDim.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int kPerWarp = kObsBinsPerCta / (kObsThreads / 32);
+    constexpr int kBinsPerCta = kPerWarp * (kObsThreads / 32);
     const bool bad = a.model_flag[b] != 0;
     const float* F = a.flux + (size_t)b * a.flux_stride;
     const double add = a.addvar ? a.addvar[b] : 0.0;
     double chi2 = 0.0;
-    const int j0 = chunk * kObsBinsPerCta + warp * kPerWarp;
+    const int j0 = chunk * kBinsPerCta + warp * kPerWarp;
 #pragma unroll 2
     for (int j = j0; j < min(j0 + kPerWarp, a.J); ++j) {
         const int p0 = a.row_ptr[j], len = a.row_ptr[j + 1] - p0;
@@ -129,29 +132,44 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
             if (bad) acc = __int_as_float(0x7fc00000);
             if (a.spectra) a.spectra[(size_t)b * a.J + j] = acc;
             if (a.logl) {
+                // every bin's term is rounded on its own and then added (explicit _rn intrinsics: no contraction into an
+                // FMA with the running sum), so the two variants of this kernel give bitwise the same logL
                 const double r = a.obs[j] - (double)acc;
+                double term;
                 if (a.addvar) {                       // Eq. 23: the normalisation depends on the model too
                     const double s2 = a.var[j] + add;
-                    chi2 += r * r / (2.0 * s2) + 0.5 * log(2.0 * kPi * s2);
+                    term = __dadd_rn(__ddiv_rn(__dmul_rn(r, r), __dmul_rn(2.0, s2)), __dmul_rn(0.5, log(__dmul_rn(2.0 * kPi, s2))));
                 } else {
-                    chi2 += r * r * a.inv2var[j];
+                    term = __dmul_rn(__dmul_rn(r, r), a.inv2var[j]);
                 }
+                chi2 = __dadd_rn(chi2, term);
             }
         }
     }
     if (!a.logl) return;
-    if (lane == 0) warp_sum[warp] = chi2;
+    // chi-square is summed in GROUPS of 8 consecutive bins, in bin order, and the groups in group order: a warp's own
+    // sum is a group when it owns 8 bins; with one bin per warp the CTA's 8 bins are a group.  Same grouping in both
+    // variants, so logL does not depend on which one ran.
+    const int n_groups = (a.J + 7) / 8;
+    if (kPerWarp == 8) {
+        const int g = chunk * (kObsThreads / 32) + warp;
+        if (lane == 0 && g < n_groups) a.partial[(size_t)b * n_groups + g] = chi2;
+    } else if (lane == 0) {
+        warp_sum[warp] = chi2;
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double s = 0.0;
-        for (int w = 0; w < kObsThreads / 32; ++w) s += warp_sum[w];
-        a.partial[(size_t)b * n_chunks + chunk] = s;
+        if (kPerWarp != 8) {
+            double s = 0.0;
+            for (int w = 0; w < kObsThreads / 32; ++w) s += warp_sum[w];
+            a.partial[(size_t)b * n_groups + chunk] = s;
+        }
         __threadfence();
         ticket = atomicAdd(&a.arrived[b], 1u);
         if (ticket == (unsigned)n_chunks - 1) {          // every chunk of this model is in `partial`
             __threadfence();
             double t = 0.0;
-            for (int c = 0; c < n_chunks; ++c) t += __ldcg(&a.partial[(size_t)b * n_chunks + c]);
+            for (int c = 0; c < n_groups; ++c) t += __ldcg(&a.partial[(size_t)b * n_groups + c]);
             a.logl[b] = bad ? -CUDART_INF : (a.addvar ? -t : a.logl_const - t);
             a.arrived[b] = 0;
         }

@@ -1,0 +1,315 @@
+// rt_seg.cuh -- fused steps 1-4, LEVEL-PARALLEL variant for small batches
+// (the paper's own usage is one model per likelihood call).
+//
+// With a handful of models there are only B * N_nu / 64 warps of work if every warp walks all L
+// levels (fewer than two per SM for one model), and each level costs a chain of dependent
+// latencies: the staged kernel needs 0.11 ms for ONE model.  But the layer update of Eq. 4,
+//     I <- e^{-D} I + (beta S_l + gamma S_{l-1}),
+// is an affine map of the incoming intensity, and affine maps compose associatively.  So the
+// level loop is cut into chunks: one CTA = one model x one 64-wavenumber tile, warp c = chunk c
+// of the layers.  Every warp integrates its chunk for an UNKNOWN incoming state, i.e. it carries,
+// per angle, the pair (Psi, C) of  H_out = Psi H_in + C  (H = (I - S)/mu as in rt_slab.cuh; Psi is
+// the chunk's transmission, C its own emission), and one warp then chains the ~15 pairs bottom-up
+// and forms the flux of Eq. 8-9.  All terms are the ones of the sequential recursion; only the
+// order of the floating-point operations differs.
+//
+// Table access: with so few models a table row is used by one warp only, so nothing is shared
+// between warps.  Every warp walks the table cells of its own levels (the cell walk of rt_slab.cuh)
+// and fetches the rows of a cell's NEW corners (2 S + C rows of 256 B) with cp.async into a private
+// shared-memory buffer one cell change AHEAD, so the L2 latency of a fetch is hidden behind the
+// levels of the current cell.  Only the rows the models touch are read at all.
+#pragma once
+#include "common.cuh"
+#include "rt_slab.cuh"
+
+namespace helios {
+
+constexpr int kSegMaxChunks = 16;       // warps per CTA
+constexpr int kSegMaxLen = 32;          // layers per chunk (L <= 16 * 32 + 1; longer atmospheres use the staged kernel)
+
+struct SegArgs {
+    const float* sigma;       // DEVICE [S][nT][nP][stride]
+    const float* cia;         // DEVICE [C][nT][stride]
+    long long stride;
+    int S, C, nT, nP, nNu, L, B;
+    const float* rec;         // DEVICE [B][L][kSlabRecFloats]   (staged-kernel records, common.cuh)
+    const float* model_x;     // DEVICE [B][x_floats]
+    int x_floats;
+    const float* model_scale;
+    const int* model_flag;
+    const int* lvl_ip;        // DEVICE [L] pressure cell of each level
+    double nu0, dnu;
+    float* flux;              // DEVICE [B][flux_stride]
+    long long flux_stride;
+    int n_chunks, chunk_len;  // chunk c owns the layers 1 + c len .. min(L - 1, (c + 1) len)  (layer j: levels j-1, j)
+};
+
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+
+// A "half" of a warp's row buffer holds the 2 S + C rows one cell change brings in: for species s the two rows
+// 2 s and 2 s + 1 (two pressure nodes of one temperature node, or two temperature nodes of one pressure node),
+// then one CIA row per pair.  fetch_half issues the copies (16 B per lane and instruction), mix_half reduces them.
+__device__ __forceinline__ void fetch_half(uint32_t dst, const float* n00, size_t dsecond, size_t srow, int S,
+                                           const float* cia, size_t crow, int C, int lane) {
+    const int n_chunks16 = (2 * S + C) * 16;             // 16-byte pieces
+    for (int ch = lane; ch < n_chunks16; ch += 32) {
+        const int r = ch >> 4, off = (ch & 15) * 4;
+        const float* src = r < 2 * S ? n00 + (size_t)(r >> 1) * srow + (size_t)(r & 1) * dsecond + off
+                                     : cia + (size_t)(r - 2 * S) * crow + off;
+        cp_async_16(dst + (uint32_t)(r * kSlabTile + off) * 4, src);
+    }
+}
+__device__ __forceinline__ void mix_half(uint32_t src, const float* x, int S, int C, int lane, float2& ga, float2& gb, float2& gc) {
+    ga = make_float2(0.0f, 0.0f); gb = ga; gc = ga;
+    const uint32_t q = src + lane * 8;
+#pragma unroll 4
+    for (int s = 0; s < S; ++s) {
+        const float2 xs = bc2(x[s]);
+        ga = __ffma2_rn(xs, lds_f2(q + (2 * s) * kSlabTile * 4), ga);
+        gb = __ffma2_rn(xs, lds_f2(q + (2 * s + 1) * kSlabTile * 4), gb);
+    }
+    for (int c = 0; c < C; ++c) gc = __ffma2_rn(bc2(x[S + c]), lds_f2(q + (2 * S + c) * kSlabTile * 4), gc);
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// One angle of one layer for the pair (Psi, C).  C takes the step of the sequential recursion (angle_step of
+// rt_slab.cuh: ex2 form for thick lanes, q-free polynomial form for thin ones), Psi the homogeneous part of the
+// same step:  Psi <- e Psi  or  Psi <- Psi - dtau P_k(dtau) Psi.
+template <int A, int K>
+__device__ __forceinline__ void angle_step_seg(float2& Cc, float2& Psi, float2 dtau, float2 ndtau, float2 q, float2 dS) {
+    constexpr double mu = kGLmu[A - 1][K];
+    constexpr float c_exp = (float)(kLog2e / mu), thr = (float)(0.25 * mu);
+    constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                    p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+    const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+    const float2 bigC = __ffma2_rn(e, Cc, __ffma2_rn(neg2(e), q, q));
+    const float2 bigP = __fmul2_rn(e, Psi);
+    float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+    P = __ffma2_rn(dtau, P, bc2(p2));
+    P = __ffma2_rn(dtau, P, bc2(p1));
+    P = __ffma2_rn(dtau, P, bc2(p0));
+    const float2 smallC = __ffma2_rn(P, __ffma2_rn(ndtau, Cc, dS), Cc);
+    const float2 smallP = __ffma2_rn(__fmul2_rn(ndtau, P), Psi, Psi);
+    Cc = make_float2(dtau.x < thr ? smallC.x : bigC.x, dtau.y < thr ? smallC.y : bigC.y);
+    Psi = make_float2(dtau.x < thr ? smallP.x : bigP.x, dtau.y < thr ? smallP.y : bigP.y);
+}
+template <int A, int K0>
+__device__ __forceinline__ void seg_angles(float2 (&Cc)[A], float2 (&Psi)[A], float2 dtau, float2 ndtau, float2 q, float2 dS) {
+    if constexpr (K0 < A) {
+        angle_step_seg<A, K0>(Cc[K0], Psi[K0], dtau, ndtau, q, dS);
+        seg_angles<A, K0 + 1>(Cc, Psi, dtau, ndtau, q, dS);
+    }
+}
+
+// shared memory: [n_chunks][A][2][64] (Psi, C) | [64] S_top | [n_chunks][2][2 S + C][64] row buffers | [x_floats] x |
+//                [n_chunks][chunk_len + 1] records + cells
+__host__ __device__ inline size_t seg_smem_bytes(int A, int n_chunks, int chunk_len, int x_floats, int S, int C) {
+    return sizeof(float) * ((size_t)n_chunks * A * 2 * kSlabTile + kSlabTile + (size_t)n_chunks * 2 * (2 * S + C) * kSlabTile +
+                            x_floats + (size_t)n_chunks * (chunk_len + 1) * (kSlabRecFloats + 4));
+}
+
+template <int A>
+__global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
+    extern __shared__ __align__(16) float seg_smem[];
+    float* ex = seg_smem;
+    float* stop = ex + (size_t)a.n_chunks * A * 2 * kSlabTile;
+    float* rows = stop + kSlabTile;
+    const int half_rows = 2 * a.S + a.C;
+    float* xs = rows + (size_t)a.n_chunks * 2 * half_rows * kSlabTile;
+    float* recs = xs + a.x_floats;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int b = blockIdx.x, tile = blockIdx.y;
+    for (int i = threadIdx.x; i < a.x_floats; i += blockDim.x) xs[i] = a.model_x[(size_t)b * a.x_floats + i];
+
+    // layers j0 .. j1-1 of this chunk need the levels j0-1 .. j1-1
+    const int j0 = 1 + warp * a.chunk_len, j1 = min(a.L, j0 + a.chunk_len);
+    const int n_lev = j1 > j0 ? j1 - j0 + 1 : 0;
+    float* rw = recs + (size_t)warp * (a.chunk_len + 1) * (kSlabRecFloats + 4);     // records, then the pressure cells
+    int* ipw = reinterpret_cast<int*>(rw + (a.chunk_len + 1) * kSlabRecFloats);
+    {
+        const float4* src = reinterpret_cast<const float4*>(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats);
+        for (int i = lane; i < n_lev * (kSlabRecFloats / 4); i += 32) reinterpret_cast<float4*>(rw)[i] = __ldg(src + i);
+        for (int i = lane; i < n_lev; i += 32) ipw[i] = __ldg(a.lvl_ip + j0 - 1 + i);
+    }
+    __syncthreads();
+
+    const int inu = tile * kSlabTile + 2 * lane;
+    const double nu_d0 = a.nu0 + a.dnu * (double)inu, nu_d1 = a.nu0 + a.dnu * (double)(inu + 1);
+    const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
+    const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
+    const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
+    const size_t prow = (size_t)a.stride, trow = prow * a.nP, srow = trow * a.nT;   // floats between p nodes / T nodes / species
+    const size_t crow = prow * a.nT;                                                // floats between CIA pairs
+    const float* sig_l = a.sigma + (size_t)tile * kSlabTile;     // first float of the tile in a row (rows are padded to the tile)
+    const float* cia_l = a.cia + (size_t)tile * kSlabTile;
+
+    float2 Cc[A], Psi[A];
+#pragma unroll
+    for (int k = 0; k < A; ++k) { Cc[k] = make_float2(0.0f, 0.0f); Psi[k] = make_float2(1.0f, 1.0f); }
+    float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
+    float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
+    const uint32_t half0 = smem_u32(rows) + (uint32_t)warp * 2 * half_rows * kSlabTile * 4, half1 = half0 + half_rows * kSlabTile * 4;
+    auto cell_iT = [&](int i) { return __float_as_int(rw[i * kSlabRecFloats + 9]); };
+    // what the change into the cell of level i brings in, relative to the cell (iT0, ip0): 1 colder, 2 hotter,
+    // 3 next pressure cell upwards, 0 anything else (all four corners)
+    auto change_kind = [&](int iT0, int ip0, int iT1, int ip1) {
+        return ip1 == ip0 ? (iT1 == iT0 - 1 ? 1 : (iT1 == iT0 + 1 ? 2 : 0)) : ((iT1 == iT0 && ip1 == ip0 - 1) ? 3 : 0);
+    };
+    auto issue = [&](int kind, int iT1, int ip1) {          // asynchronous fetch of the new corners of cell (iT1, ip1)
+        const float* n00 = sig_l + iT1 * trow + ip1 * prow;
+        const float* c0 = cia_l + iT1 * prow;
+        if (kind == 1) fetch_half(half0, n00, prow, srow, a.S, c0, crow, a.C, lane);                       // T row iT1
+        else if (kind == 2) fetch_half(half0, n00 + trow, prow, srow, a.S, c0 + prow, crow, a.C, lane);    // T row iT1 + 1
+        else if (kind == 3) fetch_half(half0, n00, trow, srow, a.S, c0, crow, 0, lane);                    // p node ip1, both T rows
+        else {
+            fetch_half(half0, n00, prow, srow, a.S, c0, crow, a.C, lane);
+            fetch_half(half1, n00 + trow, prow, srow, a.S, c0 + prow, crow, a.C, lane);
+        }
+        cp_async_commit();
+    };
+    int cur_iT = 0, cur_ip = 0, nxt = n_lev, nxt_kind = 0;
+    auto look_ahead = [&](int i) {                           // first level after i in another cell, and its fetch
+        int j = i + 1;
+        while (j < n_lev && cell_iT(j) == cur_iT && ipw[j] == cur_ip) ++j;
+        nxt = j;
+        if (j < n_lev) { nxt_kind = change_kind(cur_iT, cur_ip, cell_iT(j), ipw[j]); issue(nxt_kind, cell_iT(j), ipw[j]); }
+    };
+    if (n_lev > 0) { nxt = 0; nxt_kind = 0; issue(0, cell_iT(0), ipw[0]); }
+
+    for (int i = 0; i < n_lev; ++i) {
+        const float4 r0 = reinterpret_cast<const float4*>(rw)[3 * i], r1 = reinterpret_cast<const float4*>(rw)[3 * i + 1],
+                     r2 = reinterpret_cast<const float4*>(rw)[3 * i + 2];
+        if (i == nxt) {                       // warp-uniform: the level lies in another table cell; its rows have been fetched
+            cp_async_wait_all();
+            __syncwarp();
+            float2 unused;
+            if (nxt_kind == 1) {              // one cell colder
+                G10 = G00; G11 = G01; Gc1 = Gc0;
+                mix_half(half0, xs, a.S, a.C, lane, G00, G01, Gc0);
+            } else if (nxt_kind == 2) {       // one cell hotter
+                G00 = G10; G01 = G11; Gc0 = Gc1;
+                mix_half(half0, xs, a.S, a.C, lane, G10, G11, Gc1);
+            } else if (nxt_kind == 3) {       // next pressure cell upwards, same temperature cell
+                G01 = G00; G11 = G10;
+                mix_half(half0, xs, a.S, 0, lane, G00, G10, unused);
+            } else {
+                mix_half(half0, xs, a.S, a.C, lane, G00, G01, Gc0);
+                mix_half(half1, xs, a.S, a.C, lane, G10, G11, Gc1);
+            }
+            cur_iT = __float_as_int(r2.y); cur_ip = ipw[i];
+            __syncwarp();                     // every lane has read the buffer before the next fetch overwrites it
+            look_ahead(i);
+        }
+        float2 chi = __fmul2_rn(bc2(r0.x), G00);
+        chi = __ffma2_rn(bc2(r0.y), G01, chi);
+        chi = __ffma2_rn(bc2(r0.z), G10, chi);
+        chi = __ffma2_rn(bc2(r0.w), G11, chi);
+        chi = __ffma2_rn(bc2(r1.x), Gc0, chi);
+        chi = __ffma2_rn(bc2(r1.y), Gc1, chi);
+        // S_l = B_nu(T_l) = c1 nu^3 E / (1 - E), E = 2^(-a nu), a nu carried as a two-float product (as rt_slab.cuh)
+        const float2 ah = bc2(r1.z);
+        const float2 pr = __fmul2_rn(ah, nu);
+        float2 rr = __ffma2_rn(ah, nu, neg2(pr));
+        rr = __ffma2_rn(bc2(r1.w), nu, rr);
+        rr = __ffma2_rn(ah, nu_lo, rr);
+        const float2 E0 = make_float2(ex2_approx(-pr.x), ex2_approx(-pr.y));
+        const float2 E = __ffma2_rn(__fmul2_rn(E0, bc2(-0.69314718056f)), rr, E0);
+        const float2 om = __fadd2_rn(bc2(1.0f), neg2(E));
+        const float2 Sl = __fmul2_rn(c1nu3, __fmul2_rn(E, make_float2(rcp_approx(om.x), rcp_approx(om.y))));
+        if (i > 0) {
+            const float2 dtau = __ffma2_rn(__fadd2_rn(chi, chi_prev), bc2(r2.x), bc2(r2.z));
+            const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
+            const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
+            seg_angles<A, 0>(Cc, Psi, dtau, neg2(dtau), q, dS);
+        }
+        chi_prev = chi; S_prev = Sl;
+    }
+
+    // hand the pair of every angle to the combining warp
+    if (warp < a.n_chunks) {
+#pragma unroll
+        for (int k = 0; k < A; ++k) {
+            reinterpret_cast<float2*>(ex + ((size_t)(warp * A + k) * 2 + 0) * kSlabTile)[lane] = Psi[k];
+            reinterpret_cast<float2*>(ex + ((size_t)(warp * A + k) * 2 + 1) * kSlabTile)[lane] = Cc[k];
+        }
+        if (j1 == a.L && n_lev > 0) reinterpret_cast<float2*>(stop)[lane] = S_prev;      // the chunk that holds the top level
+    }
+    __syncthreads();
+    if (warp != 0 || inu >= a.nNu) return;
+
+    float2 H[A];
+#pragma unroll
+    for (int k = 0; k < A; ++k) H[k] = make_float2(0.0f, 0.0f);       // bottom boundary: I = S_0 (R11)
+    for (int c = 0; c < a.n_chunks; ++c) {
+#pragma unroll
+        for (int k = 0; k < A; ++k) {
+            const float2 psi = reinterpret_cast<const float2*>(ex + ((size_t)(c * A + k) * 2 + 0) * kSlabTile)[lane];
+            const float2 cc = reinterpret_cast<const float2*>(ex + ((size_t)(c * A + k) * 2 + 1) * kSlabTile)[lane];
+            H[k] = __ffma2_rn(psi, H[k], cc);
+        }
+    }
+    float* out = a.flux + (size_t)b * a.flux_stride + inu;
+    const bool two = inu + 1 < a.nNu;
+    if (a.model_flag[b]) {
+        out[0] = __int_as_float(0x7fc00000);
+        if (two) out[1] = __int_as_float(0x7fc00000);
+        return;
+    }
+    const float2 acc = flux_sum<A>(H, reinterpret_cast<const float2*>(stop)[lane], std::make_integer_sequence<int, A>{});
+    const float scale = a.model_scale[b];
+    out[0] = scale * acc.x;
+    if (two) out[1] = scale * acc.y;
+}
+
+struct SegPlan {
+    bool ok = false;
+    int n_chunks = 0, chunk_len = 0;
+    size_t smem = 0;
+};
+
+// Chunking depends on the number of levels only, so a model's result does not depend on the batch it is in.
+inline SegPlan seg_plan(int L, int A, int S, int C, int x_floats, size_t smem_optin) {
+    SegPlan p;
+    if (L < 2 || A < 1 || A > kMaxAngles) return p;
+    const int layers = L - 1;
+    int len = (layers + kSegMaxChunks - 1) / kSegMaxChunks;
+    if (len < 4) len = layers < 4 ? layers : 4;       // a chunk re-evaluates its lower boundary level: keep that under 25 %
+    if (len > kSegMaxLen) return p;
+    p.chunk_len = len;
+    p.n_chunks = (layers + len - 1) / len;
+    p.smem = seg_smem_bytes(A, p.n_chunks, len, x_floats, S, C);
+    p.ok = p.smem <= smem_optin;
+    return p;
+}
+
+template <int A>
+inline cudaError_t launch_rt_seg_a(const SegArgs& a, size_t smem, cudaStream_t stream) {
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(k_rt_seg<A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    const dim3 grid(a.B, (a.nNu + kSlabTile - 1) / kSlabTile);
+    k_rt_seg<A><<<grid, a.n_chunks * 32, smem, stream>>>(a);
+    return cudaGetLastError();
+}
+
+inline cudaError_t launch_rt_seg(int A, const SegArgs& a, size_t smem, cudaStream_t stream) {
+    switch (A) {
+        case 1: return launch_rt_seg_a<1>(a, smem, stream);
+        case 2: return launch_rt_seg_a<2>(a, smem, stream);
+        case 3: return launch_rt_seg_a<3>(a, smem, stream);
+        case 4: return launch_rt_seg_a<4>(a, smem, stream);
+        case 5: return launch_rt_seg_a<5>(a, smem, stream);
+        case 6: return launch_rt_seg_a<6>(a, smem, stream);
+        case 7: return launch_rt_seg_a<7>(a, smem, stream);
+        case 8: return launch_rt_seg_a<8>(a, smem, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace helios

@@ -39,6 +39,16 @@ constexpr int kSlabTile = 64;       // wavenumbers per CTA (one 256 B row segmen
 constexpr int kSlabMaxRing = 8;
 constexpr uint32_t kMbarSuspendNs = 20000;   // try_wait suspend-time hint: sleep in hardware instead of polling
 
+// One segment of the plane schedule with everything that depends on the ring depth NB worked out on the host
+// (slot = load index mod NB, parity = (load index / NB) & 1): the kernel does no integer division.
+struct __align__(16) SlabSeg {
+    int l_begin, l_end;             // levels [l_begin, l_end)
+    int hi, lo;                     // slot | parity << 8 of the loads holding plane ip+1 / plane ip
+    int shifted;                    // 1: this segment's upper plane is the previous segment's lower plane
+    int rel_slot, rel_count;        // slots to release when the segment is done: rel_slot, rel_slot + 1, ... (mod NB)
+    int pad;
+};
+
 struct SlabArgs {
     int S, C, nT, nNu, L, B;
     const float* rec;               // DEVICE [B][L][kSlabRecFloats]
@@ -49,10 +59,8 @@ struct SlabArgs {
     double nu0, dnu;
     float* flux;                    // DEVICE [B][flux_stride]
     long long flux_stride;
-    // plane schedule (helios_set_atmosphere)
-    const int* seg_lbegin;          // DEVICE [n_seg + 1] first level of each segment
-    const int* seg_hi;              // DEVICE [n_seg] load index holding plane ip+1
-    const int* seg_lo;              // DEVICE [n_seg] load index holding plane ip
+    // plane schedule (helios_set_atmosphere), resolved for this launch's ring depth
+    const SlabSeg* seg;             // DEVICE [n_seg]
     const int* load_ip;             // DEVICE [n_loads] pressure node of each load, in issue order
     int n_seg, n_loads;
     int ring;                       // NB, number of plane slots
@@ -80,6 +88,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t"
         "}" ::"r"(smem_u32(bar)), "r"(parity), "r"(kMbarSuspendNs) : "memory");
+}
+// The producer's wait for a free slot: it has a whole segment of compute (microseconds) to refill it, so it sleeps
+// between polls instead of competing with the compute warps of its scheduler for issue slots.
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
+    for (;;) {
+        uint32_t done;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity), "r"(kMbarSuspendNs) : "memory");
+        if (done) return;
+        __nanosleep(400);
+    }
 }
 // TMA: one box of the 4-D table view {nu, ip, iT, s} / the 3-D CIA view {nu, iT, c} -> shared memory
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
@@ -276,9 +299,10 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
                     tma_load_3d(cia_s + (size_t)c * a.nT * kSlabTile, &tm_cia, cia_bar, nu_first, 0, c);
             }
             if (a.S > 0) {
-                for (int e = 0; e < a.n_loads; ++e) {
-                    const int slot = e % NB, use = e / NB;
-                    if (use > 0) mbar_wait(&empty[slot], (uint32_t)((use - 1) & 1));
+                int slot = 0, use = 0;
+                for (int e = 0; e < a.n_loads; ++e, ++slot) {
+                    if (slot == NB) { slot = 0; ++use; }
+                    if (use > 0) mbar_wait_backoff(&empty[slot], (uint32_t)((use - 1) & 1));
                     const int ip = a.load_ip[e];
                     float* dst = planes + (size_t)slot * plane_floats;
                     mbar_expect_tx(&full[slot], (uint32_t)(sizeof(float) * plane_floats));
@@ -317,22 +341,20 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     for (int k = 0; k < A; ++k) H[k] = make_float2(0.0f, 0.0f);
     float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
     float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
-    int released = 0, cur_iT = -2, prev_lo = -1;
+    int cur_iT = -2;
 
     if (a.C > 0) mbar_wait(cia_bar, 0);
 
     for (int seg = 0; seg < a.n_seg; ++seg) {
-        const int l_begin = a.seg_lbegin[seg], l_end = a.seg_lbegin[seg + 1];
+        const int4 sg0 = __ldg(reinterpret_cast<const int4*>(a.seg + seg)), sg1 = __ldg(reinterpret_cast<const int4*>(a.seg + seg) + 1);
+        const int l_begin = sg0.x, l_end = sg0.y;
         uint32_t pLo = planes_a, pHi = planes_a;
-        bool shifted = false;                 // the previous segment's lower plane is this one's upper plane
+        const bool shifted = sg1.x != 0;      // the previous segment's lower plane is this one's upper plane
         if (a.S > 0) {
-            const int eHi = a.seg_hi[seg], eLo = a.seg_lo[seg];
-            mbar_wait(&full[eHi % NB], (uint32_t)((eHi / NB) & 1));
-            mbar_wait(&full[eLo % NB], (uint32_t)((eLo / NB) & 1));
-            pHi += (uint32_t)(eHi % NB) * plane_bytes;
-            pLo += (uint32_t)(eLo % NB) * plane_bytes;
-            shifted = eHi == prev_lo;
-            prev_lo = eLo;
+            mbar_wait(&full[sg0.z & 0xff], (uint32_t)(sg0.z >> 8));
+            mbar_wait(&full[sg0.w & 0xff], (uint32_t)(sg0.w >> 8));
+            pHi += (uint32_t)(sg0.z & 0xff) * plane_bytes;
+            pLo += (uint32_t)(sg0.w & 0xff) * plane_bytes;
         }
         bool fresh = true;
         for (int l = l_begin; l < l_end; ++l, rp += 3) {
@@ -411,13 +433,13 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             }
             chi_prev = chi; S_prev = Sl;
         }
-        if (a.S > 0 && seg + 1 < a.n_seg) {
+        if (a.S > 0 && sg1.z > 0) {
             // slots holding loads older than the next segment's are free for the producer
-            const int next_first = min(a.seg_hi[seg + 1], a.seg_lo[seg + 1]);
             __syncwarp();
-            if (lane == 0)
-                for (int e = released; e < next_first; ++e) mbar_arrive(&empty[e % NB]);
-            released = max(released, next_first);
+            if (lane == 0) {
+                int slot = sg1.y;
+                for (int i = 0; i < sg1.z; ++i) { mbar_arrive(&empty[slot]); slot = slot + 1 == NB ? 0 : slot + 1; }
+            }
         }
     }
 

@@ -37,7 +37,7 @@ def _helios(wl):
     return h
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_distance_inflation_and_cloud(torch_cuda, oracle, wl1, kernel):
     """All three extras at once, in the documented order d, epsilon, (log tau_c, log p_top, log phi)."""
     import paper_1910_01070_b200 as pkg

@@ -130,7 +130,7 @@ def _record(tag, **kv):
         pass
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_config0_tiny(torch_cuda, oracle, wl0, kernel):
     ref = oracle.forward_workload(wl0, want_flux=True)
     spec, logl, flux, st = _run(torch_cuda, wl0, wl0.params, kernel)
@@ -140,7 +140,7 @@ def test_config0_tiny(torch_cuda, oracle, wl0, kernel):
     assert st["n_clamped"] == ref["n_clamped"] * 2          # forward_batch + forward_highres
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_config1_medium_all_models(torch_cuda, oracle, wl1, kernel):
     ref = oracle.forward_workload(wl1, want_flux=True)
     spec, logl, flux, st = _run(torch_cuda, wl1, wl1.params, kernel)
@@ -151,7 +151,7 @@ def test_config1_medium_all_models(torch_cuda, oracle, wl1, kernel):
     assert st["n_clamped"] == ref["n_clamped"] * 2
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 @pytest.mark.parametrize("cfg_index", [1, 2])
 def test_logl_near_truth_absolute_tolerance(torch_cuda, oracle, wl1, wl2, kernel, cfg_index):
     wl = {1: wl1, 2: wl2}[cfg_index]
@@ -236,7 +236,7 @@ def test_logl_near_truth_config3(torch_cuda, oracle, wl3):
             max_reduced_chi2=float(red_chi2.max()), n_models=4)
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_batch_invariants(torch_cuda, wl1, kernel):
     """Permuting models permutes outputs; a model's result does not depend on the batch
     it is in; repeated runs are bitwise identical."""
@@ -252,7 +252,7 @@ def test_batch_invariants(torch_cuda, wl1, kernel):
     assert np.array_equal(spec_r, spec) and np.array_equal(logl_r, logl)
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_ragged_sizes_and_edge_cases(torch_cuda, oracle, kernel):
     """Wavenumber count not a multiple of any tile, odd level count, 1..3 angles,
     single species without CIA, CIA only, bins narrower than a grid cell, no
@@ -380,11 +380,12 @@ def test_auto_falls_back_to_the_direct_kernel_when_planes_do_not_fit(torch_cuda,
     h.close()
 
 
+@pytest.mark.parametrize("kernel", [2, 3], ids=["slab", "levelpar"])
 @pytest.mark.parametrize("seed", range(10))
-def test_random_shapes_staged_kernel(torch_cuda, oracle, seed):
-    """Random table / atmosphere shapes through the staged kernel: pressure grids denser than the
-    levels (segments that skip table cells, two new planes per segment), two-node grids, two levels,
-    one to eight angles, batches that do not fill a CTA, ring wrap-around with many planes."""
+def test_random_shapes_staged_kernel(torch_cuda, oracle, seed, kernel):
+    """Random table / atmosphere shapes through the staged and the level-parallel kernel: pressure grids denser
+    than the levels (segments that skip table cells, two new planes per segment), two-node grids, two levels
+    (one chunk of one layer), one to eight angles, batches that do not fill a CTA, ring wrap-around with many planes."""
     import paper_1910_01070_b200 as pkg
     torch = torch_cuda
     rng = np.random.default_rng(1000 + seed)
@@ -415,7 +416,7 @@ def test_random_shapes_staged_kernel(torch_cuda, oracle, seed):
     h.load_opacity(T_grid, lp_grid, nu0, dnu, sigma, cia)
     h.set_atmosphere(L, 200.0, 2e-4, K, A, 2.3, 0.17, 1.0)
     h.set_observation(edges, obs, err, inst)
-    h.set_kernel(2)
+    h.set_kernel(kernel)
     p = torch.as_tensor(params, device="cuda:0")
     spec, logl = h.forward_batch(p)
     flux = h.forward_highres(p)
@@ -458,7 +459,7 @@ def test_n_params_is_checked(torch_cuda, wl1):
     h.close()
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["direct", "slab"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 def test_unphysical_models_are_rejected(torch_cuda, oracle, wl1, kernel):
     """Finite but unphysical parameter vectors (R31) give logL = -inf (never NaN) and NaN
     spectra, are counted, and leave their neighbours bit-identical; the oracle applies the same rule."""
@@ -482,3 +483,25 @@ def test_unphysical_models_are_rejected(torch_cuda, oracle, wl1, kernel):
     assert np.array_equal(spec[good], spec0[good]) and np.array_equal(logl[good], logl0[good])
     assert np.array_equal(flux[good], flux0[good])
     assert _relerr(spec[good], ref["spectra"][good]) <= TOL_FLUX
+
+
+def test_small_batches_take_the_level_parallel_kernel_and_agree_with_the_staged_one(torch_cuda, oracle, wl2):
+    """configs[2] tables with B = 1, 2, 4 in the launch configuration bench.py times for small batches
+    (kernel = auto -> level-parallel up to the measured crossover B = 4): every model against the oracle, and against
+    the staged kernel's result for the same vectors (different operation order: agreement to a few ulp, not bitwise)."""
+    params = wl2.params[:8]
+    ref = oracle.forward_workload(wl2, params=params, want_flux=True)
+    spec_s, logl_s, flux_s, _ = _run(torch_cuda, wl2, params, kernel=2)
+    for B in (1, 2, 4, 8):
+        spec, logl, flux, _ = _run(torch_cuda, wl2, params[:B], kernel=0)
+        assert _relerr(flux, ref["flux_hr"][:B]) <= TOL_FLUX
+        assert _relerr(spec, ref["spectra"][:B]) <= TOL_FLUX
+        _check_logl(wl2, logl, {"spectra": ref["spectra"][:B], "logl": ref["logl"][:B]}, spec)
+        assert _relerr(flux, flux_s[:B]) <= 5e-6
+        forced = _run(torch_cuda, wl2, params[:B], kernel=3 if B <= 4 else 2)
+        assert np.array_equal(forced[0], spec) and np.array_equal(forced[2], flux)     # which kernel auto really took
+    near = W.near_truth_params(wl2.cfg, 4)
+    refn = oracle.forward_workload(wl2, params=near)
+    specn, logln, _, _ = _run(torch_cuda, wl2, near, kernel=0, highres=False)
+    assert np.max(np.abs(logln - refn["logl"])) <= TOL_LOGL_ABS
+    _record("configs[2] near truth, B = 4 (level-parallel)", max_abs_dlogl=float(np.max(np.abs(logln - refn["logl"]))), n_models=4)
