@@ -21,6 +21,8 @@ HELIOS_PTRS_ON_DEVICE = 1
 HELIOS_OPT_KERNEL = 1
 HELIOS_OPT_MODELS_PER_CTA = 2
 HELIOS_OPT_TIMING = 3
+HELIOS_OPT_NU_ORDER = 4
+NU_ORDER_GRID, NU_ORDER_OPACITY = 0, 1
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB, KERNEL_LEVEL_PARALLEL = 0, 1, 2, 3
 HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD = 1, 2, 4
 
@@ -350,6 +352,10 @@ class Helios:
     def set_observation(self, bin_edges, obs=None, obs_err=None, inst_sigma=None):
         helios_set_observation(self.ctx, bin_edges, obs, obs_err, inst_sigma)
         self.n_bins = len(bin_edges) - 1
+
+    def set_nu_order(self, order: int):
+        """Column order of the resident tables for the NEXT load_opacity (NU_ORDER_OPACITY is the default)."""
+        helios_set_option(self.ctx, HELIOS_OPT_NU_ORDER, order)
 
     def set_kernel(self, which: int, models_per_cta: int = 0):
         helios_set_option(self.ctx, HELIOS_OPT_KERNEL, which)

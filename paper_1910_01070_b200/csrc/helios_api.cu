@@ -34,8 +34,9 @@ struct helios_ctx {
     long long stride = 0;               // padded row length, floats
     double nu0 = 0, dnu = 0;
     std::vector<double> T_grid, lp_grid;
-    float* d_sigma = nullptr;           // [S][nT][nP][stride]
+    float* d_sigma = nullptr;           // [S][nT][nP][stride]   columns in the order of d_nu_index
     float* d_cia = nullptr;             // [C][nT][stride]
+    int* d_nu_index = nullptr;          // [stride] wavenumber grid index held by every table column (>= nNu: padding)
     double* d_Tgrid = nullptr;
 
     // ---- atmosphere
@@ -59,6 +60,7 @@ struct helios_ctx {
     bool have_tmaps = false;
     CUtensorMap tm_sigma{}, tm_cia{};
     size_t smem_optin = 0, smem_sm = 0;
+    SlabSmemCache slab_smem;
 
     // ---- observation
     bool have_obs = false, have_data = false;
@@ -78,7 +80,7 @@ struct helios_ctx {
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
     // ---- options / statistics
-    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0;
+    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0, opt_nu_order = 1;
     static constexpr int kTimingRing = 64;
     cudaEvent_t ev[kTimingRing][4] = {};
     bool ev_has_obs[kTimingRing] = {};
@@ -121,7 +123,7 @@ static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
 }
 
 static void free_all(helios_ctx* c) {
-    dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid);
+    dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid); dfree(c->d_nu_index);
     dfree(c->d_lvl_p); dfree(c->d_lvl_elem); dfree(c->d_lvl_lw); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
     dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
     dfree(c->d_seg); dfree(c->d_load_ip);
@@ -203,6 +205,40 @@ static bool build_tensor_maps(helios_ctx* c) {
     }
     c->have_tmaps = true;
     return true;
+}
+
+// Column order of the resident tables.  The kernels own 64 adjacent table columns per warp and take warp-uniform
+// shortcuts when all of them are optically thin (or thick) in a layer, so columns of similar opacity should sit
+// next to each other -- and on a fine grid adjacent WAVENUMBERS are not: line cores and wings alternate.  The
+// columns are therefore sorted once, at load time, by a reference opacity: the cross-sections at one table node
+// (middle temperature, a low pressure where the lines are sharp), grouped by the species that dominates the
+// column and ordered by its cross-section within the group.  Every kernel reads nu_index[column] for the
+// wavenumber and writes its flux to that grid point, so the order is invisible outside the library.
+static void opacity_order(const std::vector<std::vector<float>>& ref_rows, int nNu, std::vector<int>& order) {
+    order.resize(nNu);
+    for (int i = 0; i < nNu; ++i) order[i] = i;
+    const int S = (int)ref_rows.size();
+    if (S == 0) return;
+    std::vector<int> dom(nNu, 0);
+    std::vector<float> val(nNu, 0.0f);
+    for (int i = 0; i < nNu; ++i) {
+        int best = 0;
+        for (int s = 1; s < S; ++s) if (ref_rows[s][i] > ref_rows[best][i]) best = s;
+        dom[i] = best; val[i] = ref_rows[best][i];
+    }
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
+        if (dom[x] != dom[y]) return dom[x] < dom[y];
+        return val[x] < val[y];
+    });
+}
+
+// dst[row][j] = src[row][nu_index[j]] for j < nNu, 0 in the padding: rows of nNu floats -> rows of `stride` floats
+__global__ void k_gather_rows(float* dst, const float* src, const int* nu_index, int nNu, long long stride, long long rows) {
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= stride) return;
+    const int g = nu_index[j];
+    for (long long r = blockIdx.y; r < rows; r += gridDim.y)
+        dst[r * stride + j] = (j < nNu) ? src[r * (long long)nNu + g] : 0.0f;
 }
 
 // One micro-benchmark: one block of 1024 threads per SM, timed with CUDA events on the context's stream (the
@@ -294,6 +330,9 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24)
                 return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16, 20 or 24");
             c->opt_models_per_cta = value; return HELIOS_OK;
+        case HELIOS_OPT_NU_ORDER:
+            if (value != 0 && value != 1) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_NU_ORDER must be 0 (grid order) or 1 (opacity order)");
+            c->opt_nu_order = value; return HELIOS_OK;
         case HELIOS_OPT_TIMING:
             c->opt_timing = value ? 1 : 0; c->timed_calls = 0;
             if (value && !c->ev_created) {
@@ -319,26 +358,53 @@ int helios_load_opacity(helios_ctx* c, int S, int nT, const double* T_grid, int 
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     c->have_tables = c->have_atmo = c->have_obs = c->have_data = false;
-    dfree(c->d_sigma); dfree(c->d_cia);
+    dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_nu_index);
     c->S = S; c->C = C; c->nT = nT; c->nP = nP; c->nNu = nNu; c->nu0 = nu0; c->dnu = dnu;
     c->stride = ((long long)nNu + kSlabTile - 1) / kSlabTile * kSlabTile;   // rows padded to the staged kernel's tile (256 B)
     c->T_grid.assign(T_grid, T_grid + nT);
     c->lp_grid.assign(lp_grid, lp_grid + nP);
-    const cudaMemcpyKind kind = (flags & HELIOS_PTRS_ON_DEVICE) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    const bool on_device = (flags & HELIOS_PTRS_ON_DEVICE) != 0;
     const size_t rows_s = (size_t)nT * nP;
+    // column order (HELIOS_OPT_NU_ORDER): reference rows at the middle temperature node and a low-pressure node
+    std::vector<int> order;
+    {
+        std::vector<std::vector<float>> ref;
+        if (c->opt_nu_order == 1 && S > 0) {
+            const int iT_ref = nT / 2, ip_ref = (int)std::lround(0.375 * (nP - 1));
+            ref.assign(S, std::vector<float>(nNu));
+            for (int s = 0; s < S; ++s)
+                CU_TRY(c, cudaMemcpy(ref[s].data(), sigma[s] + ((size_t)iT_ref * nP + ip_ref) * nNu, sizeof(float) * nNu,
+                                     on_device ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost));
+        }
+        opacity_order(ref, nNu, order);
+        order.resize((size_t)c->stride);
+        for (long long j = nNu; j < c->stride; ++j) order[j] = (int)j;      // padding columns: >= nNu, never written out
+        CU_TRY(c, upload(c->d_nu_index, order, c->stream));
+    }
+    // upload: rows of nNu floats -> padded rows in column order (through a device staging slab when the source is on the host)
+    float* d_stage = nullptr;
+    struct Stage { float*& p; ~Stage() { dfree(p); } } stage_guard{d_stage};
+    const size_t slab_rows = std::max(rows_s, (size_t)nT);
+    if (!on_device) CU_TRY(c, cudaMalloc(&d_stage, sizeof(float) * slab_rows * nNu));
+    auto put = [&](float* dst, const float* src, size_t rows) -> cudaError_t {
+        const float* dsrc = src;
+        if (!on_device) {
+            cudaError_t e = cudaMemcpyAsync(d_stage, src, sizeof(float) * rows * nNu, cudaMemcpyHostToDevice, c->stream);
+            if (e != cudaSuccess) return e;
+            dsrc = d_stage;
+        }
+        const dim3 grid((unsigned)((c->stride + 255) / 256), (unsigned)std::min<size_t>(rows, 1024));
+        k_gather_rows<<<grid, 256, 0, c->stream>>>(dst, dsrc, c->d_nu_index, nNu, c->stride, (long long)rows);
+        c->n_launches += 1;
+        return cudaGetLastError();
+    };
     if (S > 0) {
         CU_TRY(c, cudaMalloc(&c->d_sigma, sizeof(float) * (size_t)S * rows_s * c->stride));
-        CU_TRY(c, cudaMemsetAsync(c->d_sigma, 0, sizeof(float) * (size_t)S * rows_s * c->stride, c->stream));
-        for (int s = 0; s < S; ++s)
-            CU_TRY(c, cudaMemcpy2DAsync(c->d_sigma + (size_t)s * rows_s * c->stride, sizeof(float) * c->stride, sigma[s],
-                                        sizeof(float) * nNu, sizeof(float) * nNu, rows_s, kind, c->stream));
+        for (int s = 0; s < S; ++s) CU_TRY(c, put(c->d_sigma + (size_t)s * rows_s * c->stride, sigma[s], rows_s));
     }
     if (C > 0) {
         CU_TRY(c, cudaMalloc(&c->d_cia, sizeof(float) * (size_t)C * nT * c->stride));
-        CU_TRY(c, cudaMemsetAsync(c->d_cia, 0, sizeof(float) * (size_t)C * nT * c->stride, c->stream));
-        for (int k = 0; k < C; ++k)
-            CU_TRY(c, cudaMemcpy2DAsync(c->d_cia + (size_t)k * nT * c->stride, sizeof(float) * c->stride, cia[k],
-                                        sizeof(float) * nNu, sizeof(float) * nNu, nT, kind, c->stream));
+        for (int k = 0; k < C; ++k) CU_TRY(c, put(c->d_cia + (size_t)k * nT * c->stride, cia[k], (size_t)nT));
     }
     CU_TRY(c, upload(c->d_Tgrid, c->T_grid, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
@@ -666,7 +732,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         SegArgs ga{};
         ga.sigma = c->d_sigma; ga.cia = c->d_cia; ga.stride = c->stride; ga.S = c->S; ga.C = c->C; ga.nT = c->nT; ga.nP = c->nP;
         ga.nNu = c->nNu; ga.L = c->L; ga.B = B; ga.rec = c->d_rec; ga.model_x = c->d_model_x; ga.x_floats = pa.x_floats;
-        ga.model_scale = c->d_scale; ga.model_flag = c->d_flag; ga.lvl_ip = c->d_lvl_ip; ga.nu0 = c->nu0; ga.dnu = c->dnu;
+        ga.model_scale = c->d_scale; ga.model_flag = c->d_flag; ga.lvl_ip = c->d_lvl_ip; ga.nu_index = c->d_nu_index; ga.nu0 = c->nu0; ga.dnu = c->dnu;
         ga.flux = flux; ga.flux_stride = flux_stride; ga.n_chunks = seg.n_chunks; ga.chunk_len = seg.chunk_len;
         cudaError_t e = launch_rt_seg(c->A, ga, seg.smem, c->stream);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "level-parallel kernel launch failed: %s", cudaGetErrorString(e));
@@ -678,11 +744,11 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         SlabArgs sa{};
         sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nNu = c->nNu; sa.L = c->L; sa.B = B;
         sa.rec = c->d_rec; sa.model_x = c->d_model_x; sa.x_floats = pa.x_floats;
-        sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu;
+        sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu; sa.nu_index = c->d_nu_index;
         sa.flux = flux; sa.flux_stride = flux_stride;
         sa.seg = c->d_seg + (size_t)(plan.ring - 1) * c->n_seg; sa.load_ip = c->d_load_ip;
         sa.n_seg = c->n_seg; sa.n_loads = c->n_loads; sa.ring = plan.ring; sa.ang = c->ang;
-        cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->stream);
+        cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->slab_smem, c->stream);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "staged kernel launch failed: %s", cudaGetErrorString(e));
         c->n_launches += 1;
         stamp(c, 2);
@@ -690,7 +756,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     }
     DirectArgs da{};
     da.sigma = c->d_sigma; da.cia = c->d_cia; da.S = c->S; da.C = c->C; da.nT = c->nT; da.nP = c->nP; da.nNu = c->nNu;
-    da.L = c->L; da.stride = c->stride; da.rec = c->d_rec; da.rec_floats = rf; da.model_scale = c->d_scale;
+    da.L = c->L; da.stride = c->stride; da.nu_index = c->d_nu_index; da.rec = c->d_rec; da.rec_floats = rf; da.model_scale = c->d_scale;
     da.model_flag = c->d_flag; da.nu0 = c->nu0; da.dnu = c->dnu; da.flux = flux; da.flux_stride = flux_stride; da.ang = c->ang;
     const size_t smem = sizeof(float) * (size_t)c->L * rf;     // the direct kernel keeps one model's records in shared memory
     if (smem > c->smem_optin)

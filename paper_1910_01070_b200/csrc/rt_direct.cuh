@@ -14,6 +14,7 @@ struct DirectArgs {
     const float* cia;        // DEVICE [C][nT][stride]
     int S, C, nT, nP, nNu, L;
     long long stride;        // padded row length (floats)
+    const int* nu_index;     // DEVICE [stride]  wavenumber grid index of every table column (helios_load_opacity)
     const float* rec;        // DEVICE [B][L][rec_floats]
     int rec_floats;
     const float* model_scale;
@@ -34,12 +35,13 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
     for (int i = threadIdx.x; i < a.L * a.rec_floats; i += kDirectThreads) srec[i] = grec[i];
     __syncthreads();
 
-    const int inu = blockIdx.x * kDirectThreads + threadIdx.x;
+    const int inu = blockIdx.x * kDirectThreads + threadIdx.x;     // column of the (re-ordered) table
     if (inu >= a.nNu) return;
-    float* out = a.flux + (size_t)b * a.flux_stride + inu;
+    const int gnu = a.nu_index[inu];                                // its wavenumber grid point
+    float* out = a.flux + (size_t)b * a.flux_stride + gnu;
     if (a.model_flag[b]) { *out = __int_as_float(0x7fc00000); return; }
 
-    const double nu_d = a.nu0 + a.dnu * (double)inu;
+    const double nu_d = a.nu0 + a.dnu * (double)gnu;
     const float nu = (float)nu_d;
     const float nu_lo = (float)(nu_d - (double)nu);
     const float c1nu3 = (float)(kC1 * nu_d * nu_d * nu_d);

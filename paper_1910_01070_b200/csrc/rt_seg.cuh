@@ -38,16 +38,13 @@ struct SegArgs {
     const float* model_scale;
     const int* model_flag;
     const int* lvl_ip;        // DEVICE [L] pressure cell of each level
+    const int* nu_index;      // DEVICE [stride]  wavenumber grid index of every table column (helios_load_opacity)
     double nu0, dnu;
     float* flux;              // DEVICE [B][flux_stride]
     long long flux_stride;
     int n_chunks, chunk_len;  // chunk c owns the layers 1 + c len .. min(L - 1, (c + 1) len)  (layer j: levels j-1, j)
 };
 
-__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 
 // A "half" of a warp's row buffer holds the 2 S + C rows one cell change brings in: for species s the two rows
 // 2 s and 2 s + 1 (two pressure nodes of one temperature node, or two temperature nodes of one pressure node),
@@ -73,7 +70,6 @@ __device__ __forceinline__ void mix_half(uint32_t src, const float* x, int S, in
     }
     for (int c = 0; c < C; ++c) gc = __ffma2_rn(bc2(x[S + c]), lds_f2(q + (2 * S + c) * kSlabTile * 4), gc);
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // One angle of one layer for the pair (Psi, C).  C takes the step of the sequential recursion (angle_step of
 // rt_slab.cuh: ex2 form for thick lanes, q-free polynomial form for thin ones), Psi the homogeneous part of the
@@ -139,7 +135,8 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
     __syncthreads();
 
     const int inu = tile * kSlabTile + 2 * lane;
-    const double nu_d0 = a.nu0 + a.dnu * (double)inu, nu_d1 = a.nu0 + a.dnu * (double)(inu + 1);
+    const int2 gnu = __ldg(reinterpret_cast<const int2*>(a.nu_index + inu));
+    const double nu_d0 = a.nu0 + a.dnu * (double)gnu.x, nu_d1 = a.nu0 + a.dnu * (double)gnu.y;
     const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
     const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
     const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
@@ -240,7 +237,7 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
         if (j1 == a.L && n_lev > 0) reinterpret_cast<float2*>(stop)[lane] = S_prev;      // the chunk that holds the top level
     }
     __syncthreads();
-    if (warp != 0 || inu >= a.nNu) return;
+    if (warp != 0) return;
 
     float2 H[A];
 #pragma unroll
@@ -253,17 +250,17 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
             H[k] = __ffma2_rn(psi, H[k], cc);
         }
     }
-    float* out = a.flux + (size_t)b * a.flux_stride + inu;
-    const bool two = inu + 1 < a.nNu;
+    float* out = a.flux + (size_t)b * a.flux_stride;
+    const bool one = gnu.x < a.nNu, two = gnu.y < a.nNu;
     if (a.model_flag[b]) {
-        out[0] = __int_as_float(0x7fc00000);
-        if (two) out[1] = __int_as_float(0x7fc00000);
+        if (one) out[gnu.x] = __int_as_float(0x7fc00000);
+        if (two) out[gnu.y] = __int_as_float(0x7fc00000);
         return;
     }
     const float2 acc = flux_sum<A>(H, reinterpret_cast<const float2*>(stop)[lane], std::make_integer_sequence<int, A>{});
     const float scale = a.model_scale[b];
-    out[0] = scale * acc.x;
-    if (two) out[1] = scale * acc.y;
+    if (one) out[gnu.x] = scale * acc.x;
+    if (two) out[gnu.y] = scale * acc.y;
 }
 
 struct SegPlan {

@@ -57,6 +57,7 @@ struct SlabArgs {
     const float* model_scale;
     const int* model_flag;
     double nu0, dnu;
+    const int* nu_index;            // DEVICE [stride]  wavenumber grid index of every table column (helios_load_opacity)
     float* flux;                    // DEVICE [B][flux_stride]
     long long flux_stride;
     // plane schedule (helios_set_atmosphere), resolved for this launch's ring depth
@@ -114,6 +115,17 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, ui
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
         ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ float4 lds_f4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
 }
 
 __device__ __forceinline__ float2 bc2(float v) { return make_float2(v, v); }
@@ -260,10 +272,21 @@ struct LayerLimits {
     static constexpr unsigned all_thin = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][0]));
 };
 
-// shared memory: [ring][S*nT*64] planes | [C*nT*64] CIA | [NW][x_floats] | mbarriers
+// Level records are staged per warp: blocks of kRecBlk levels, double-buffered, copied with cp.async one block ahead
+// (a record is read once per wavenumber tile, and every new 32-byte sector of it was an L2 round trip at the top of
+// the level iteration: 16 % of all warp stall samples at configs[3]).
+#ifndef HELIOS_SLAB_RECBLK
+#define HELIOS_SLAB_RECBLK 8
+#endif
+constexpr int kRecBlk = HELIOS_SLAB_RECBLK;          // power of two; 0 = records straight from global memory
+constexpr int kRecRingFloats = 2 * kRecBlk * kSlabRecFloats;
+constexpr int kRecBlkDiv = kRecBlk > 0 ? kRecBlk : 1;
+
+// shared memory: [ring][S*nT*64] planes | [C*nT*64] CIA | [NW][x_floats] | [NW][2][kRecBlk] records | mbarriers
 __host__ __device__ inline size_t slab_plane_floats(int S, int nT) { return (size_t)S * nT * kSlabTile; }
 __host__ __device__ inline size_t slab_fixed_bytes(int C, int nT, int NW, int x_floats) {
-    return sizeof(float) * ((size_t)C * nT * kSlabTile + (size_t)NW * x_floats) + 8 * (2 * kSlabMaxRing + 1) + 128;
+    return sizeof(float) * ((size_t)C * nT * kSlabTile + (size_t)NW * x_floats + (size_t)NW * kRecRingFloats) +
+           8 * (2 * kSlabMaxRing + 1) + 128;
 }
 
 template <int A, int NW, int MINB>
@@ -274,7 +297,8 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     float* planes = reinterpret_cast<float*>(smem_raw);
     float* cia_s = planes + (size_t)a.ring * plane_floats;
     float* xs_s = cia_s + (size_t)a.C * a.nT * kSlabTile;
-    uint64_t* full = reinterpret_cast<uint64_t*>(xs_s + NW * a.x_floats);
+    float* rec_s = xs_s + NW * a.x_floats;
+    uint64_t* full = reinterpret_cast<uint64_t*>(rec_s + NW * kRecRingFloats);
     uint64_t* empty = full + kSlabMaxRing;
     uint64_t* cia_bar = empty + kSlabMaxRing;
 
@@ -322,8 +346,10 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     for (int i = lane; i < a.x_floats; i += 32) xw[i] = a.model_x[(size_t)b * a.x_floats + i];
     __syncwarp();
 
+    // the lane's two table columns and the wavenumber grid points they hold (the table's nu axis is re-ordered)
     const int inu = tile * kSlabTile + 2 * lane;
-    const double nu_d0 = a.nu0 + a.dnu * (double)inu, nu_d1 = a.nu0 + a.dnu * (double)(inu + 1);
+    const int2 gnu = __ldg(reinterpret_cast<const int2*>(a.nu_index + inu));
+    const double nu_d0 = a.nu0 + a.dnu * (double)gnu.x, nu_d1 = a.nu0 + a.dnu * (double)gnu.y;
     const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
     const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
     const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
@@ -331,6 +357,15 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     const uint32_t spB = a.nT * kRowB;        // bytes between species in a plane
     const float* rec_b = a.rec + (size_t)b * a.L * kSlabRecFloats;
     const float4* rp = reinterpret_cast<const float4*>(rec_b);
+    const uint32_t rb_a = smem_u32(rec_s + warp * kRecRingFloats);
+    const int n_rec16 = a.L * (kSlabRecFloats / 4);                    // 16-byte pieces of this model's records
+    auto stage_block = [&](int blk) {                                 // levels blk kRecBlk .. + kRecBlk - 1 -> half blk & 1
+        const int piece = blk * kRecBlk * (kSlabRecFloats / 4) + lane;
+        if (lane < kRecBlk * (kSlabRecFloats / 4) && piece < n_rec16)
+            cp_async_16(rb_a + (uint32_t)(((blk & 1) * kRecBlk * (kSlabRecFloats / 4) + lane) * 16), rp + piece);
+        cp_async_commit();
+    };
+    if (kRecBlk > 0) stage_block(0);
     const uint32_t planes_a = smem_u32(planes) + lane * 8;   // shared-memory byte addresses of this lane's pair
     const uint32_t cia_a = smem_u32(cia_s) + lane * 8;
     const uint32_t xw_a = smem_u32(xw), xc_a = xw_a + a.S * 4;
@@ -357,8 +392,19 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
             pLo += (uint32_t)(sg0.w & 0xff) * plane_bytes;
         }
         bool fresh = true;
-        for (int l = l_begin; l < l_end; ++l, rp += 3) {
-            const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2);
+        for (int l = l_begin; l < l_end; ++l) {
+            float4 r0, r1, r2;
+            if (kRecBlk > 0) {
+                if ((l & (kRecBlkDiv - 1)) == 0) {          // this block has landed (issued a block ago); fetch the next one
+                    cp_async_wait_all();
+                    __syncwarp();
+                    stage_block(l / kRecBlkDiv + 1);
+                }
+                const uint32_t ra = rb_a + (uint32_t)(l & (2 * kRecBlkDiv - 1)) * (kSlabRecFloats * 4);
+                r0 = lds_f4(ra); r1 = lds_f4(ra + 16); r2 = lds_f4(ra + 32);
+            } else {
+                r0 = __ldg(rp + 3 * l); r1 = __ldg(rp + 3 * l + 1); r2 = __ldg(rp + 3 * l + 2);
+            }
             const int iT = __float_as_int(r2.y);
             if (fresh || iT != cur_iT) {      // warp-uniform: the model is in another table cell
                 const uint32_t lo = pLo + iT * kRowB, hi = pHi + iT * kRowB, qc = cia_a + iT * kRowB;
@@ -443,19 +489,19 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
         }
     }
 
-    if (!model_valid || inu >= a.nNu) return;
-    float* out = a.flux + (size_t)b * a.flux_stride + inu;
-    const bool two = inu + 1 < a.nNu;
+    if (!model_valid) return;
+    float* out = a.flux + (size_t)b * a.flux_stride;       // written in grid order: columns of the padding map to >= nNu
+    const bool one = gnu.x < a.nNu, two = gnu.y < a.nNu;
     if (a.model_flag[b]) {
-        out[0] = __int_as_float(0x7fc00000);
-        if (two) out[1] = __int_as_float(0x7fc00000);
+        if (one) out[gnu.x] = __int_as_float(0x7fc00000);
+        if (two) out[gnu.y] = __int_as_float(0x7fc00000);
         return;
     }
     // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = mu_k H_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
     const float2 acc = flux_sum<A>(H, S_prev, std::make_integer_sequence<int, A>{});
     const float scale = a.model_scale[b];
-    out[0] = scale * acc.x;
-    if (two) out[1] = scale * acc.y;
+    if (one) out[gnu.x] = scale * acc.x;
+    if (two) out[gnu.y] = scale * acc.y;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -464,7 +510,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 struct SlabPlan {
     bool ok = false;
     int NW = 0, ring = 0;
-    size_t smem = 0;
+    size_t smem = 0, smem_optin = 0;
 };
 
 // Picks the models-per-CTA variant and the ring depth that fit the shared memory of one SM.
@@ -487,51 +533,55 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
         const int need = n_loads >= 3 ? 3 : (n_loads > 0 ? n_loads : 1);
         if (plane && ring < need) continue;
         if (ring < 1) ring = 1;
-        p.ok = true; p.NW = nw; p.ring = ring; p.smem = fixed + plane * ring;
+        p.ok = true; p.NW = nw; p.ring = ring; p.smem = fixed + plane * ring; p.smem_optin = smem_optin;
         return p;
     }
     return p;
 }
 
+// `configured` = this CONTEXT has raised the kernel instance's dynamic shared-memory limit (a context lives on one
+// device and is used by one host thread at a time, so the flag needs no lock).  The limit is a property of the
+// function, shared by every context of the process: it is always set to the device's opt-in maximum, never to the
+// size one context happens to need, so contexts with different table shapes cannot lower it for each other.
 template <int A, int NW, int MINB>
-inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, size_t smem,
-                                    cudaStream_t stream) {
-    static size_t configured[64] = {};   // per kernel instance and device; setting it again is harmless, so no lock
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dev < 0 || dev >= 64 || smem > configured[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
+                                    bool& configured, cudaStream_t stream) {
+    const size_t smem = p.smem;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_optin);
         if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) configured[dev] = smem;
+        configured = true;
     }
     const dim3 grid((a.B + NW - 1) / NW, (a.nNu + kSlabTile - 1) / kSlabTile);
     k_rt_slab<A, NW, MINB><<<grid, (NW + 1) * 32, smem, stream>>>(tms, tmc, a);
     return cudaGetLastError();
 }
 
+struct SlabSmemCache { bool configured[kMaxAngles + 1][4] = {}; };     // [A][models-per-CTA variant], one per context
+
 template <int A>
 inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
-                                    cudaStream_t stream) {
+                                    SlabSmemCache& cache, cudaStream_t stream) {
     switch (p.NW) {
-        case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p.smem, stream);
-        case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p.smem, stream);
-        case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p.smem, stream);
-        case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p.smem, stream);
+        case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p, cache.configured[A][0], stream);
+        case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p, cache.configured[A][1], stream);
+        case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p, cache.configured[A][2], stream);
+        case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p, cache.configured[A][3], stream);
         default: return cudaErrorInvalidValue;
     }
 }
 
 inline cudaError_t launch_rt_slab(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
-                                  cudaStream_t stream) {
+                                  SlabSmemCache& cache, cudaStream_t stream) {
     switch (a.ang.n) {
-        case 1: return launch_rt_slab_a<1>(tms, tmc, a, p, stream);
-        case 2: return launch_rt_slab_a<2>(tms, tmc, a, p, stream);
-        case 3: return launch_rt_slab_a<3>(tms, tmc, a, p, stream);
-        case 4: return launch_rt_slab_a<4>(tms, tmc, a, p, stream);
-        case 5: return launch_rt_slab_a<5>(tms, tmc, a, p, stream);
-        case 6: return launch_rt_slab_a<6>(tms, tmc, a, p, stream);
-        case 7: return launch_rt_slab_a<7>(tms, tmc, a, p, stream);
-        case 8: return launch_rt_slab_a<8>(tms, tmc, a, p, stream);
+        case 1: return launch_rt_slab_a<1>(tms, tmc, a, p, cache, stream);
+        case 2: return launch_rt_slab_a<2>(tms, tmc, a, p, cache, stream);
+        case 3: return launch_rt_slab_a<3>(tms, tmc, a, p, cache, stream);
+        case 4: return launch_rt_slab_a<4>(tms, tmc, a, p, cache, stream);
+        case 5: return launch_rt_slab_a<5>(tms, tmc, a, p, cache, stream);
+        case 6: return launch_rt_slab_a<6>(tms, tmc, a, p, cache, stream);
+        case 7: return launch_rt_slab_a<7>(tms, tmc, a, p, cache, stream);
+        case 8: return launch_rt_slab_a<8>(tms, tmc, a, p, cache, stream);
         default: return cudaErrorInvalidValue;
     }
 }
