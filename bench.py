@@ -294,11 +294,16 @@ def run_gpu(args):
     for _ in range(max(args.warmup, 3)):
         step_device()
     h.stats(reset=True)
-    h.set_timing(True)
     ms, clocks, per_step = timed(step_device, args.steps, ClockSampler(local) if rank == 0 else None)
-    stage = h.stage_ms()
     st = h.stats(reset=True)
+    # per-stage device times: a separate, untimed pass with the library's own CUDA events between the kernels (those
+    # events serialise the kernels, which the timed region above launches as programmatic dependents)
+    h.set_timing(True)
+    for _ in range(max(3, min(args.steps, 64 // n_calls))):
+        step_device()
+    stage = h.stage_ms()
     h.set_timing(False)
+    h.stats(reset=True)
     for _ in range(2):
         step_host()
     ms_host, _, per_step_host = timed(step_host, args.steps)

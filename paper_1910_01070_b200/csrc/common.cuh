@@ -41,7 +41,7 @@ __host__ __device__ inline int direct_rec_floats(int S, int C) { return (4 * S +
 //   0..3  n 2^-32 {(1-t)(1-u), (1-t)u, t(1-u), t u}   weights of G at (iT,ip), (iT,ip+1), (iT+1,ip), (iT+1,ip+1)
 //   4..5  am^2 {(1-t), t}                               weights of the CIA mix at iT, iT+1
 //   6..7  planck_a high / low      8  hdz of the layer BELOW the level (levels l-1, l; 0 at level 0)      9  iT (int bits)
-//   10  dtau_cloud of the layer below      11  unused
+//   10  dtau_cloud of the layer below      11  cell-walk schedule (int bits): kind | distance to the next cell change << 8 (prep.cuh)
 // Per-model vector, slab_x_floats(S, C) floats: x_s 2^32 (S values), then x_H2 x_c (C values).
 constexpr int kSlabRecFloats = 12;
 constexpr float kSlabXScale = 4294967296.0f;   // 2^32: keeps x_s sigma_s far above the fp32 denormal range
@@ -90,6 +90,25 @@ constexpr double kGLw[8][8] = {
     {0.05061426814518853, 0.11119051722668721, 0.15685332293894344, 0.18134189168918083, 0.18134189168918083, 0.15685332293894344, 0.11119051722668721, 0.05061426814518853},
 };
 __host__ __device__ constexpr double cpow(double b, int e) { double r = 1.0; for (int i = 0; i < e; ++i) r *= b; return r; }
+
+// Programmatic dependent launch (sm_90+): the three kernels of a call are launched back to back with the
+// programmatic-stream-serialization attribute, so the next kernel's CTAs are scheduled and run their prologue while
+// the previous kernel drains; pdl_wait() blocks until the previous kernel has completed and its writes are visible
+// (a no-op when the kernel was launched without the attribute).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, bool pdl,
+                                 Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 __device__ __forceinline__ float ex2_approx(float x) {
     float y;

@@ -57,10 +57,12 @@ struct helios_ctx {
     int n_seg = 0, n_loads = 0;
     SlabSeg* d_seg = nullptr;           // [kSlabMaxRing][n_seg]: the schedule resolved for every ring depth
     int* d_load_ip = nullptr;
-    bool have_tmaps = false;
+    bool have_tmaps = false, have_seg_maps = false;
     CUtensorMap tm_sigma{}, tm_cia{};
+    SegMaps seg_maps{};                 // level-parallel kernel: boxes of one cell change (rt_seg.cuh)
     size_t smem_optin = 0, smem_sm = 0;
     SlabSmemCache slab_smem;
+    SegSmemCache seg_smem;
 
     // ---- observation
     bool have_obs = false, have_data = false;
@@ -172,10 +174,10 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 static bool build_tensor_maps(helios_ctx* c) {
-    c->have_tmaps = false;
+    c->have_tmaps = c->have_seg_maps = false;
     std::memset(&c->tm_sigma, 0, sizeof c->tm_sigma);
     std::memset(&c->tm_cia, 0, sizeof c->tm_cia);
-    if (c->nT > 256) return false;
+    std::memset(&c->seg_maps, 0, sizeof c->seg_maps);
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess ||
@@ -185,6 +187,33 @@ static bool build_tensor_maps(helios_ctx* c) {
     }
     encode_tiled_fn encode = (encode_tiled_fn)fn;
     const cuuint64_t row = (cuuint64_t)c->stride * sizeof(float);
+    // level-parallel kernel: all species at two pressure nodes of one temperature node / two temperature nodes of one
+    // pressure node; all CIA pairs at one temperature node
+    {
+        bool ok = true;
+        cuuint32_t estr[4] = {1, 1, 1, 1};
+        if (c->S > 0) {
+            cuuint64_t dims[4] = {(cuuint64_t)c->stride, (cuuint64_t)c->nP, (cuuint64_t)c->nT, (cuuint64_t)c->S};
+            cuuint64_t strides[3] = {row, row * c->nP, row * c->nP * c->nT};
+            cuuint32_t box_p2[4] = {(cuuint32_t)kSlabTile, 2, 1, (cuuint32_t)c->S}, box_t2[4] = {(cuuint32_t)kSlabTile, 1, 2, (cuuint32_t)c->S};
+            ok = ok && encode(&c->seg_maps.p2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->d_sigma, dims, strides, box_p2, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            ok = ok && encode(&c->seg_maps.t2, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, c->d_sigma, dims, strides, box_t2, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        }
+        if (c->C > 0) {
+            cuuint64_t dims[3] = {(cuuint64_t)c->stride, (cuuint64_t)c->nT, (cuuint64_t)c->C};
+            cuuint64_t strides[2] = {row, row * c->nT};
+            cuuint32_t box[3] = {(cuuint32_t)kSlabTile, 1, (cuuint32_t)c->C};
+            ok = ok && encode(&c->seg_maps.c, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, c->d_cia, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+        }
+        c->have_seg_maps = ok;
+    }
+    if (c->nT > 256) return false;        // the staged kernel's box holds every temperature node of a plane
     if (c->S > 0) {
         cuuint64_t dims[4] = {(cuuint64_t)c->stride, (cuuint64_t)c->nP, (cuuint64_t)c->nT, (cuuint64_t)c->S};
         cuuint64_t strides[3] = {row, row * c->nP, row * c->nP * c->nT};
@@ -646,7 +675,12 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
     return HELIOS_OK;
 }
 
-constexpr int kSegAutoMaxBatch = 4;       // measured crossover with the staged kernel (profiles/r02_batch_sweep.md)
+// Automatic choice of the level-parallel kernel: measured crossovers with the staged kernel (profiles/r02_batch_sweep.md)
+// are B = 8..16 at configs[1] (133 tiles) and configs[2] (255 tiles), B = 4..8 at configs[3] (1329 tiles): the staged
+// kernel's time is flat up to there (its warps walk all levels in sequence), the level-parallel kernel's grows with
+// B x tiles.
+constexpr int kSegAutoMaxBatch = 8;
+constexpr long long kSegAutoMaxCtas = 6000;
 constexpr int kObsSmallBatchCtas = 592;     // 4 CTAs of 8 warps per SM on 148 SMs
 
 static SlabPlan plan_slab(const helios_ctx* c, int B) {
@@ -707,7 +741,8 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     if (c->opt_kernel == 2 && !plan.ok)
         return fail(c, HELIOS_EINVAL, "staged kernel requested but unavailable for this table shape (shared memory / TMA)");
     // level-parallel kernel: small batches (measured crossover, profiles/r02_batch_sweep.md), or on request
-    const SegPlan seg = (c->opt_kernel == 3 || (c->opt_kernel == 0 && B <= kSegAutoMaxBatch))
+    const SegPlan seg = (c->have_seg_maps && (c->opt_kernel == 3 || (c->opt_kernel == 0 && B <= kSegAutoMaxBatch &&
+                                                                  (long long)B * ((c->nNu + kSlabTile - 1) / kSlabTile) <= kSegAutoMaxCtas)))
                             ? seg_plan(c->L, c->A, c->S, c->C, slab_x_floats(c->S, c->C), c->smem_optin) : SegPlan{};
     if (c->opt_kernel == 3 && !seg.ok)
         return fail(c, HELIOS_EINVAL, "level-parallel kernel requested but unavailable for %d levels", c->L);
@@ -722,6 +757,9 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
     pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
     pa.counters = c->d_counters;
+    // programmatic dependent launch of the RT and observation kernels (common.cuh); not with stage timing, whose
+    // events between the kernels serialise them
+    const bool pdl = !c->opt_timing;
     stamp(c, 0);
     k_prep<<<B, kPrepThreads, 0, c->stream>>>(pa);
     c->n_launches += 1;
@@ -734,7 +772,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         ga.nNu = c->nNu; ga.L = c->L; ga.B = B; ga.rec = c->d_rec; ga.model_x = c->d_model_x; ga.x_floats = pa.x_floats;
         ga.model_scale = c->d_scale; ga.model_flag = c->d_flag; ga.lvl_ip = c->d_lvl_ip; ga.nu_index = c->d_nu_index; ga.nu0 = c->nu0; ga.dnu = c->dnu;
         ga.flux = flux; ga.flux_stride = flux_stride; ga.n_chunks = seg.n_chunks; ga.chunk_len = seg.chunk_len;
-        cudaError_t e = launch_rt_seg(c->A, ga, seg.smem, c->stream);
+        cudaError_t e = launch_rt_seg(c->A, c->seg_maps, ga, seg.smem, c->smem_optin, c->seg_smem, c->stream, pdl);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "level-parallel kernel launch failed: %s", cudaGetErrorString(e));
         c->n_launches += 1;
         stamp(c, 2);
@@ -748,7 +786,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         sa.flux = flux; sa.flux_stride = flux_stride;
         sa.seg = c->d_seg + (size_t)(plan.ring - 1) * c->n_seg; sa.load_ip = c->d_load_ip;
         sa.n_seg = c->n_seg; sa.n_loads = c->n_loads; sa.ring = plan.ring; sa.ang = c->ang;
-        cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->slab_smem, c->stream);
+        cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->slab_smem, c->stream, pdl);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "staged kernel launch failed: %s", cudaGetErrorString(e));
         c->n_launches += 1;
         stamp(c, 2);
@@ -766,7 +804,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
 #define HELIOS_DIRECT_CASE(N)                                                                               \
     case N:                                                                                                 \
         if (smem > 48 * 1024) CU_TRY(c, cudaFuncSetAttribute(k_rt_direct<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        k_rt_direct<N><<<grid, kDirectThreads, smem, c->stream>>>(da);                                      \
+        CU_TRY(c, launch_kernel(k_rt_direct<N>, grid, dim3(kDirectThreads), smem, c->stream, pdl, da));     \
         break;
     switch (c->A) {
         HELIOS_DIRECT_CASE(1) HELIOS_DIRECT_CASE(2) HELIOS_DIRECT_CASE(3) HELIOS_DIRECT_CASE(4)
@@ -821,12 +859,13 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     oa.partial = c->d_obs_partial; oa.arrived = c->d_obs_arrived;
     // one bin per warp while 64-bin CTAs would leave SMs idle (the choice depends on B only through this threshold;
     // kObsSmallBatchCtas is fixed, so a given (B, J) always takes the same variant)
+    const bool pdl = !c->opt_timing;
     if ((long long)B * ((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta) < kObsSmallBatchCtas)
-        k_obs_apply<1><<<dim3((c->J + 7) / 8, B), kObsThreads, 0, c->stream>>>(oa);
+        CU_TRY(c, launch_kernel(k_obs_apply<1>, dim3((c->J + 7) / 8, B), dim3(kObsThreads), 0, c->stream, pdl, oa));
     else
-        k_obs_apply<8><<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa);
+        CU_TRY(c, launch_kernel(k_obs_apply<8>, dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), dim3(kObsThreads), 0,
+                                c->stream, pdl, oa));
     c->n_launches += 1;
-    CU_TRY(c, cudaGetLastError());
     stamp(c, 3);
     if (c->opt_timing) { c->ev_has_obs[c->timed_calls % helios_ctx::kTimingRing] = true; c->timed_calls++; }
     return HELIOS_OK;

@@ -42,6 +42,7 @@ struct PrepArgs {
 constexpr int kMaxTpNodes = 5;    // order <= 4
 constexpr int kPrepThreads = 128;
 constexpr int kPrepMaxSpecies = 64;
+constexpr int kPrepMaxLevels = 4096;
 
 // Eq. 12: T(level) = sum_i T_dof[k q + i] l_i(xi).  In the ratio form the nodal temperatures are the
 // running products T_1 b_2 ... b_j (R28), rebuilt here for the element's q + 1 nodes.
@@ -62,7 +63,10 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
     __shared__ double sx[kPrepMaxSpecies];     // 10^(log10 VMR)
     __shared__ double sm[8];                   // g, x_h2, x_he, cloud tau, cloud p_top, cloud p_bot
     __shared__ int s_ok;
+    __shared__ short s_cell[kPrepMaxLevels];   // temperature cell of every level (cell-walk schedule below)
+    __shared__ double s_T[kPrepMaxLevels];     // temperature of every level (each one is needed by three levels)
     const int b = blockIdx.x, tid = threadIdx.x;
+    pdl_launch_dependents();       // the RT kernel may be scheduled now; it waits for this grid before reading the records
     const double* th = a.params + (size_t)b * a.P;
     const double* tpar = th + 2;
     const double* lvmr = th + 2 + a.NT;
@@ -111,32 +115,41 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
         }
     }
 
+    if (model_ok)
+        for (int l = tid; l < a.L; l += kPrepThreads)
+            s_T[l] = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l], a.lvl_lw + (size_t)l * kMaxTpNodes);
+    __syncthreads();
+
     bool bad_level = false;
     for (int l = tid; l < a.L; l += kPrepThreads) {
         float* rec = a.rec + ((size_t)b * a.L + l) * a.rec_floats;
         double T = 0.0, T_up = 0.0, T_dn = 0.0;
         bool ok = model_ok;
         if (ok) {
-            T = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l], a.lvl_lw + (size_t)l * kMaxTpNodes);
-            if (l + 1 < a.L) T_up = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l + 1], a.lvl_lw + (size_t)(l + 1) * kMaxTpNodes);
-            if (l > 0) T_dn = level_temperature(tpar, a.tp_order, a.tp_ratio, a.lvl_elem[l - 1], a.lvl_lw + (size_t)(l - 1) * kMaxTpNodes);
+            T = s_T[l];
+            if (l + 1 < a.L) T_up = s_T[l + 1];
+            if (l > 0) T_dn = s_T[l - 1];
             ok = T > 0.0 && isfinite(T) && (l + 1 >= a.L || (T_up > 0.0 && isfinite(T_up))) && (l == 0 || (T_dn > 0.0 && isfinite(T_dn)));
         }
         if (!ok) {
             bad_level = true;
             for (int i = 0; i < a.rec_floats; ++i) rec[i] = 0.0f;
+            s_cell[l] = 0;
             continue;
         }
         const double p = a.lvl_p_bar[l];
         // temperature cell: largest iT with T_grid[iT] <= T, clamped to [0, nT-2]
         int iT = 0;
-        for (int k = 0; k < a.nT; ++k) if (a.T_grid[k] <= T) iT = k;
-        if (iT > a.nT - 2) iT = a.nT - 2;
+        for (int hi = a.nT - 1; hi - iT > 1;) {       // bisection: T_grid[iT] <= T < T_grid[hi] (or T outside the grid)
+            const int mid = (iT + hi) >> 1;
+            if (a.T_grid[mid] <= T) iT = mid; else hi = mid;
+        }
         double t = (T - a.T_grid[iT]) / (a.T_grid[iT + 1] - a.T_grid[iT]);
         int clamped = a.lvl_pclamp[l];
         if (t < 0.0) { t = 0.0; clamped = 1; }
         if (t > 1.0) { t = 1.0; clamped = 1; }
         if (clamped) atomicAdd(&a.counters[0], 1ULL);
+        s_cell[l] = (short)iT;
         const double u = a.lvl_u[l];
         const double n = p * kBarCgs / (kBoltzmann * T);     // cm^-3
         const double am = n / kAmagat;
@@ -194,6 +207,24 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
         while (o < a.rec_floats) rec[o++] = 0.0f;
     }
     const int any_bad = __syncthreads_or(bad_level);
+    if (a.slab_layout) {
+        // Cell-walk schedule (slot 11 of the staged record, read by the level-parallel kernel): how the table cell of
+        // level l relates to the cell of level l - 1 -- 4 same cell, 1 one cell colder, 2 one cell hotter, 3 next
+        // pressure cell upwards at the same temperature cell, 0 anything else -- and the distance to the next level
+        // that lies in another cell (0: none), so that the kernel can prefetch a cell's corners without scanning.
+        for (int l = tid; l < a.L; l += kPrepThreads) {
+            int kind = 0;
+            if (l > 0) {
+                const int iT0 = s_cell[l - 1], ip0 = a.lvl_ip[l - 1], iT1 = s_cell[l], ip1 = a.lvl_ip[l];
+                kind = ip1 == ip0 ? (iT1 == iT0 ? 4 : (iT1 == iT0 - 1 ? 1 : (iT1 == iT0 + 1 ? 2 : 0)))
+                                  : ((iT1 == iT0 && ip1 == ip0 - 1) ? 3 : 0);
+            }
+            int j = l + 1;
+            while (j < a.L && s_cell[j] == s_cell[l] && a.lvl_ip[j] == a.lvl_ip[l]) ++j;
+            const int dist = j < a.L ? j - l : 0;
+            a.rec[((size_t)b * a.L + l) * a.rec_floats + 11] = __int_as_float(kind | (dist << 8));
+        }
+    }
     if (tid == 0) {
         const bool ok = model_ok && !any_bad;
         a.model_flag[b] = ok ? 0 : 1;

@@ -31,6 +31,7 @@ template <int A>
 __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
     extern __shared__ float srec[];          // [L][rec_floats]
     const int b = blockIdx.y;
+    pdl_wait();
     const float* grec = a.rec + (size_t)b * a.L * a.rec_floats;
     for (int i = threadIdx.x; i < a.L * a.rec_floats; i += kDirectThreads) srec[i] = grec[i];
     __syncthreads();
@@ -90,6 +91,7 @@ __global__ void __launch_bounds__(kDirectThreads) k_rt_direct(DirectArgs a) {
     float acc = S_prev * a.ang.wmu_sum;
 #pragma unroll
     for (int k = 0; k < A; ++k) acc = fmaf(a.ang.wmu[k], J[k], acc);
+    pdl_launch_dependents();
     *out = a.model_scale[b] * acc;
 }
 

@@ -15,16 +15,22 @@
 //
 // Table access: with so few models a table row is used by one warp only, so nothing is shared
 // between warps.  Every warp walks the table cells of its own levels (the cell walk of rt_slab.cuh)
-// and fetches the rows of a cell's NEW corners (2 S + C rows of 256 B) with cp.async into a private
-// shared-memory buffer one cell change AHEAD, so the L2 latency of a fetch is hidden behind the
-// levels of the current cell.  Only the rows the models touch are read at all.
+// and fetches the rows of a cell's NEW corners (2 S + C rows of 256 B) into a private shared-memory
+// buffer one cell change AHEAD with one or two TMA boxes (cp.async.bulk.tensor, all species at once) that
+// complete on the warp's mbarrier, so a fetch costs a dozen instructions and its HBM latency is hidden behind
+// the levels of the current cell.  Which level enters which cell, and how the new cell relates to the old
+// one, is worked out once per model by the prep kernel (record slot 11).  Only the rows the models touch
+// are read at all.
 #pragma once
 #include "common.cuh"
 #include "rt_slab.cuh"
 
 namespace helios {
 
-constexpr int kSegMaxChunks = 16;       // warps per CTA
+#ifndef HELIOS_SEG_CHUNKS
+#define HELIOS_SEG_CHUNKS 8
+#endif
+constexpr int kSegMaxChunks = HELIOS_SEG_CHUNKS;       // warps per CTA
 constexpr int kSegMaxLen = 32;          // layers per chunk (L <= 16 * 32 + 1; longer atmospheres use the staged kernel)
 
 struct SegArgs {
@@ -46,19 +52,10 @@ struct SegArgs {
 };
 
 
-// A "half" of a warp's row buffer holds the 2 S + C rows one cell change brings in: for species s the two rows
+// A warp's row buffer holds the 2 S + C rows one cell change brings in (a "half" of a cell's corners): for species s the two rows
 // 2 s and 2 s + 1 (two pressure nodes of one temperature node, or two temperature nodes of one pressure node),
-// then one CIA row per pair.  fetch_half issues the copies (16 B per lane and instruction), mix_half reduces them.
-__device__ __forceinline__ void fetch_half(uint32_t dst, const float* n00, size_t dsecond, size_t srow, int S,
-                                           const float* cia, size_t crow, int C, int lane) {
-    const int n_chunks16 = (2 * S + C) * 16;             // 16-byte pieces
-    for (int ch = lane; ch < n_chunks16; ch += 32) {
-        const int r = ch >> 4, off = (ch & 15) * 4;
-        const float* src = r < 2 * S ? n00 + (size_t)(r >> 1) * srow + (size_t)(r & 1) * dsecond + off
-                                     : cia + (size_t)(r - 2 * S) * crow + off;
-        cp_async_16(dst + (uint32_t)(r * kSlabTile + off) * 4, src);
-    }
-}
+// then one CIA row per pair.  One TMA box brings in all 2 S species rows (tensor maps of helios_api.cu:
+// box {64 nu, 2 p nodes, 1 T node, S} or {64, 1, 2, S}), another the C CIA rows; mix_half reduces a half.
 __device__ __forceinline__ void mix_half(uint32_t src, const float* x, int S, int C, int lane, float2& ga, float2& gb, float2& gc) {
     ga = make_float2(0.0f, 0.0f); gb = ga; gc = ga;
     const uint32_t q = src + lane * 8;
@@ -101,25 +98,61 @@ __device__ __forceinline__ void seg_angles(float2 (&Cc)[A], float2 (&Psi)[A], fl
     }
 }
 
-// shared memory: [n_chunks][A][2][64] (Psi, C) | [64] S_top | [n_chunks][2][2 S + C][64] row buffers | [x_floats] x |
-//                [n_chunks][chunk_len + 1] records + cells
+// The same step when every lane of the warp is on one branch for every angle (LayerLimits of rt_slab.cuh): bitwise the
+// values angle_step_seg selects.
+template <int A, int K0>
+__device__ __forceinline__ void seg_angles_thick(float2 (&Cc)[A], float2 (&Psi)[A], float2 ndtau, float2 q) {
+    if constexpr (K0 < A) {
+        constexpr float c_exp = (float)(kLog2e / kGLmu[A - 1][K0]);
+        const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+        const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+        Cc[K0] = __ffma2_rn(e, Cc[K0], __ffma2_rn(neg2(e), q, q));
+        Psi[K0] = __fmul2_rn(e, Psi[K0]);
+        seg_angles_thick<A, K0 + 1>(Cc, Psi, ndtau, q);
+    }
+}
+template <int A, int K0>
+__device__ __forceinline__ void seg_angles_thin(float2 (&Cc)[A], float2 (&Psi)[A], float2 dtau, float2 ndtau, float2 dS) {
+    if constexpr (K0 < A) {
+        constexpr double mu = kGLmu[A - 1][K0];
+        constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                        p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+        float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+        P = __ffma2_rn(dtau, P, bc2(p2));
+        P = __ffma2_rn(dtau, P, bc2(p1));
+        P = __ffma2_rn(dtau, P, bc2(p0));
+        Cc[K0] = __ffma2_rn(P, __ffma2_rn(ndtau, Cc[K0], dS), Cc[K0]);
+        Psi[K0] = __ffma2_rn(__fmul2_rn(ndtau, P), Psi[K0], Psi[K0]);
+        seg_angles_thin<A, K0 + 1>(Cc, Psi, dtau, ndtau, dS);
+    }
+}
+
+// shared memory: [n_chunks][A][2][64] (Psi, C) | [64] S_top | [n_chunks][2 S + C][64] row buffers | [x_floats] x |
+//                [n_chunks][chunk_len + 1] records + cells | [n_chunks] mbarriers
 __host__ __device__ inline size_t seg_smem_bytes(int A, int n_chunks, int chunk_len, int x_floats, int S, int C) {
-    return sizeof(float) * ((size_t)n_chunks * A * 2 * kSlabTile + kSlabTile + (size_t)n_chunks * 2 * (2 * S + C) * kSlabTile +
-                            x_floats + (size_t)n_chunks * (chunk_len + 1) * (kSlabRecFloats + 4));
+    return sizeof(float) * ((size_t)n_chunks * A * 2 * kSlabTile + kSlabTile + (size_t)n_chunks * (2 * S + C) * kSlabTile +
+                            x_floats + (size_t)n_chunks * (chunk_len + 1) * (kSlabRecFloats + 4)) + 8 * (size_t)n_chunks + 8;
 }
 
 template <int A>
-__global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
-    extern __shared__ __align__(16) float seg_smem[];
+__global__ void __launch_bounds__(kSegMaxChunks * 32, kSegMaxChunks <= 8 ? 3 : 1)
+k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUtensorMap tm_t2,
+         const __grid_constant__ CUtensorMap tm_c, SegArgs a) {
+    extern __shared__ __align__(128) float seg_smem[];
     float* ex = seg_smem;
     float* stop = ex + (size_t)a.n_chunks * A * 2 * kSlabTile;
     float* rows = stop + kSlabTile;
     const int half_rows = 2 * a.S + a.C;
-    float* xs = rows + (size_t)a.n_chunks * 2 * half_rows * kSlabTile;
+    float* xs = rows + (size_t)a.n_chunks * half_rows * kSlabTile;
     float* recs = xs + a.x_floats;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(
+        (reinterpret_cast<uintptr_t>(recs + (size_t)a.n_chunks * (a.chunk_len + 1) * (kSlabRecFloats + 4)) + 7) & ~(uintptr_t)7);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int b = blockIdx.x, tile = blockIdx.y;
+    if (lane == 0) mbar_init(&bars[warp], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    pdl_wait();                    // records, x and flags come from the prep kernel
     for (int i = threadIdx.x; i < a.x_floats; i += blockDim.x) xs[i] = a.model_x[(size_t)b * a.x_floats + i];
 
     // layers j0 .. j1-1 of this chunk need the levels j0-1 .. j1-1
@@ -127,6 +160,31 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
     const int n_lev = j1 > j0 ? j1 - j0 + 1 : 0;
     float* rw = recs + (size_t)warp * (a.chunk_len + 1) * (kSlabRecFloats + 4);     // records, then the pressure cells
     int* ipw = reinterpret_cast<int*>(rw + (a.chunk_len + 1) * kSlabRecFloats);
+    const uint32_t half0 = smem_u32(rows) + (uint32_t)warp * half_rows * kSlabTile * 4;
+    const uint32_t cia_off = (uint32_t)(2 * a.S) * kSlabTile * 4;
+    uint64_t* bar = &bars[warp];
+    uint32_t phase = 0;
+    const int nu_first = tile * kSlabTile;
+    // asynchronous fetch of new corners of cell (iT1, ip1) into the warp's buffer:
+    //   what = 1: temperature row iT1, pressure nodes ip1 and ip1 + 1, CIA row iT1      (one cell colder; first half of a new cell)
+    //   what = 2: temperature row iT1 + 1, the same                                      (one cell hotter; second half of a new cell)
+    //   what = 3: pressure node ip1, temperature rows iT1 and iT1 + 1, no CIA            (next pressure cell upwards)
+    auto issue = [&](int what, int iT1, int ip1) {
+        if (lane != 0) return;
+        const uint32_t sig_bytes = (uint32_t)(2 * a.S) * kSlabTile * 4, cia_bytes = (uint32_t)a.C * kSlabTile * 4;
+        const bool with_cia = a.C > 0 && what != 3;
+        mbar_expect_tx(bar, sig_bytes + (with_cia ? cia_bytes : 0u));
+        const int iTa = what == 2 ? iT1 + 1 : iT1;
+        if (a.S > 0) tma_load_4d(nullptr, what == 3 ? &tm_t2 : &tm_p2, bar, nu_first, ip1, iTa, 0, half0);
+        if (with_cia) tma_load_3d(nullptr, &tm_c, bar, nu_first, iTa, 0, half0 + cia_off);
+    };
+    // the chunk's first cell, straight from global memory, so that its fetch is in flight while the records are staged
+    int first_iT = 0, first_ip = 0;
+    if (lane == 0 && n_lev > 0) {
+        first_iT = __float_as_int(__ldg(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats + 9));
+        first_ip = __ldg(a.lvl_ip + j0 - 1);
+        issue(1, first_iT, first_ip);          // a new cell = two fetches (what 1 here, what 2 in the level loop)
+    }
     {
         const float4* src = reinterpret_cast<const float4*>(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats);
         for (int i = lane; i < n_lev * (kSlabRecFloats / 4); i += 32) reinterpret_cast<float4*>(rw)[i] = __ldg(src + i);
@@ -140,50 +198,24 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
     const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
     const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
     const float2 c1nu3 = make_float2((float)(kC1 * nu_d0 * nu_d0 * nu_d0), (float)(kC1 * nu_d1 * nu_d1 * nu_d1));
-    const size_t prow = (size_t)a.stride, trow = prow * a.nP, srow = trow * a.nT;   // floats between p nodes / T nodes / species
-    const size_t crow = prow * a.nT;                                                // floats between CIA pairs
-    const float* sig_l = a.sigma + (size_t)tile * kSlabTile;     // first float of the tile in a row (rows are padded to the tile)
-    const float* cia_l = a.cia + (size_t)tile * kSlabTile;
 
     float2 Cc[A], Psi[A];
 #pragma unroll
     for (int k = 0; k < A; ++k) { Cc[k] = make_float2(0.0f, 0.0f); Psi[k] = make_float2(1.0f, 1.0f); }
     float2 chi_prev = make_float2(0.0f, 0.0f), S_prev = chi_prev;
     float2 G00 = chi_prev, G01 = chi_prev, G10 = chi_prev, G11 = chi_prev, Gc0 = chi_prev, Gc1 = chi_prev;
-    const uint32_t half0 = smem_u32(rows) + (uint32_t)warp * 2 * half_rows * kSlabTile * 4, half1 = half0 + half_rows * kSlabTile * 4;
+    auto sched = [&](int i) { return __float_as_int(rw[i * kSlabRecFloats + 11]); };
     auto cell_iT = [&](int i) { return __float_as_int(rw[i * kSlabRecFloats + 9]); };
-    // what the change into the cell of level i brings in, relative to the cell (iT0, ip0): 1 colder, 2 hotter,
-    // 3 next pressure cell upwards, 0 anything else (all four corners)
-    auto change_kind = [&](int iT0, int ip0, int iT1, int ip1) {
-        return ip1 == ip0 ? (iT1 == iT0 - 1 ? 1 : (iT1 == iT0 + 1 ? 2 : 0)) : ((iT1 == iT0 && ip1 == ip0 - 1) ? 3 : 0);
-    };
-    auto issue = [&](int kind, int iT1, int ip1) {          // asynchronous fetch of the new corners of cell (iT1, ip1)
-        const float* n00 = sig_l + iT1 * trow + ip1 * prow;
-        const float* c0 = cia_l + iT1 * prow;
-        if (kind == 1) fetch_half(half0, n00, prow, srow, a.S, c0, crow, a.C, lane);                       // T row iT1
-        else if (kind == 2) fetch_half(half0, n00 + trow, prow, srow, a.S, c0 + prow, crow, a.C, lane);    // T row iT1 + 1
-        else if (kind == 3) fetch_half(half0, n00, trow, srow, a.S, c0, crow, 0, lane);                    // p node ip1, both T rows
-        else {
-            fetch_half(half0, n00, prow, srow, a.S, c0, crow, a.C, lane);
-            fetch_half(half1, n00 + trow, prow, srow, a.S, c0 + prow, crow, a.C, lane);
-        }
-        cp_async_commit();
-    };
-    int cur_iT = 0, cur_ip = 0, nxt = n_lev, nxt_kind = 0;
-    auto look_ahead = [&](int i) {                           // first level after i in another cell, and its fetch
-        int j = i + 1;
-        while (j < n_lev && cell_iT(j) == cur_iT && ipw[j] == cur_ip) ++j;
-        nxt = j;
-        if (j < n_lev) { nxt_kind = change_kind(cur_iT, cur_ip, cell_iT(j), ipw[j]); issue(nxt_kind, cell_iT(j), ipw[j]); }
-    };
-    if (n_lev > 0) { nxt = 0; nxt_kind = 0; issue(0, cell_iT(0), ipw[0]); }
+    // the level after which the rows in flight are needed, and how they relate to the current cell
+    int nxt = n_lev, nxt_kind = 0;
+    if (n_lev > 0) nxt = 0;                   // the first level's cell is in flight already
 
     for (int i = 0; i < n_lev; ++i) {
         const float4 r0 = reinterpret_cast<const float4*>(rw)[3 * i], r1 = reinterpret_cast<const float4*>(rw)[3 * i + 1],
                      r2 = reinterpret_cast<const float4*>(rw)[3 * i + 2];
         if (i == nxt) {                       // warp-uniform: the level lies in another table cell; its rows have been fetched
-            cp_async_wait_all();
-            __syncwarp();
+            mbar_wait(bar, phase);
+            phase ^= 1u;
             float2 unused;
             if (nxt_kind == 1) {              // one cell colder
                 G10 = G00; G11 = G01; Gc1 = Gc0;
@@ -194,13 +226,18 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
             } else if (nxt_kind == 3) {       // next pressure cell upwards, same temperature cell
                 G01 = G00; G11 = G10;
                 mix_half(half0, xs, a.S, 0, lane, G00, G10, unused);
-            } else {
+            } else {                          // a new cell: all four corners, in two fetches through the one buffer
                 mix_half(half0, xs, a.S, a.C, lane, G00, G01, Gc0);
-                mix_half(half1, xs, a.S, a.C, lane, G10, G11, Gc1);
+                __syncwarp();
+                issue(2, cell_iT(i), ipw[i]);
+                mbar_wait(bar, phase);
+                phase ^= 1u;
+                mix_half(half0, xs, a.S, a.C, lane, G10, G11, Gc1);
             }
-            cur_iT = __float_as_int(r2.y); cur_ip = ipw[i];
             __syncwarp();                     // every lane has read the buffer before the next fetch overwrites it
-            look_ahead(i);
+            const int dist = sched(i) >> 8;   // next level in another cell (prep.cuh), 0: none
+            nxt = dist > 0 ? i + dist : n_lev;
+            if (nxt < n_lev) { nxt_kind = sched(nxt) & 0xff; issue(nxt_kind == 0 ? 1 : nxt_kind, cell_iT(nxt), ipw[nxt]); }
         }
         float2 chi = __fmul2_rn(bc2(r0.x), G00);
         chi = __ffma2_rn(bc2(r0.y), G01, chi);
@@ -221,8 +258,16 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
         if (i > 0) {
             const float2 dtau = __ffma2_rn(__fadd2_rn(chi, chi_prev), bc2(r2.x), bc2(r2.z));
             const float2 dS = __fadd2_rn(S_prev, neg2(Sl));
-            const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
-            seg_angles<A, 0>(Cc, Psi, dtau, neg2(dtau), q, dS);
+            const float2 ndtau = neg2(dtau);
+            const unsigned d_lo = __reduce_min_sync(0xffffffffu, __float_as_uint(fminf(dtau.x, dtau.y)));
+            const unsigned d_hi = __reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(dtau.x, dtau.y)));
+            if (d_hi < LayerLimits<A>::all_thin) {
+                seg_angles_thin<A, 0>(Cc, Psi, dtau, ndtau, dS);
+            } else {
+                const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
+                if (d_lo >= LayerLimits<A>::all_thick) seg_angles_thick<A, 0>(Cc, Psi, ndtau, q);
+                else seg_angles<A, 0>(Cc, Psi, dtau, ndtau, q, dS);
+            }
         }
         chi_prev = chi; S_prev = Sl;
     }
@@ -237,6 +282,7 @@ __global__ void __launch_bounds__(kSegMaxChunks * 32) k_rt_seg(SegArgs a) {
         if (j1 == a.L && n_lev > 0) reinterpret_cast<float2*>(stop)[lane] = S_prev;      // the chunk that holds the top level
     }
     __syncthreads();
+    pdl_launch_dependents();
     if (warp != 0) return;
 
     float2 H[A];
@@ -284,27 +330,34 @@ inline SegPlan seg_plan(int L, int A, int S, int C, int x_floats, size_t smem_op
     return p;
 }
 
+// `configured`: this context has raised the instance's dynamic shared-memory limit to the opt-in maximum (see rt_slab.cuh)
+struct SegMaps { CUtensorMap p2, t2, c; };
+
 template <int A>
-inline cudaError_t launch_rt_seg_a(const SegArgs& a, size_t smem, cudaStream_t stream) {
-    if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(k_rt_seg<A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+inline cudaError_t launch_rt_seg_a(const SegMaps& m, const SegArgs& a, size_t smem, size_t smem_optin, bool& configured,
+                                   cudaStream_t stream, bool pdl) {
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_rt_seg<A>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_optin);
         if (e != cudaSuccess) return e;
+        configured = true;
     }
     const dim3 grid(a.B, (a.nNu + kSlabTile - 1) / kSlabTile);
-    k_rt_seg<A><<<grid, a.n_chunks * 32, smem, stream>>>(a);
-    return cudaGetLastError();
+    return launch_kernel(k_rt_seg<A>, grid, dim3(a.n_chunks * 32), smem, stream, pdl, m.p2, m.t2, m.c, a);
 }
 
-inline cudaError_t launch_rt_seg(int A, const SegArgs& a, size_t smem, cudaStream_t stream) {
+struct SegSmemCache { bool configured[kMaxAngles + 1] = {}; };
+
+inline cudaError_t launch_rt_seg(int A, const SegMaps& m, const SegArgs& a, size_t smem, size_t smem_optin, SegSmemCache& cache,
+                                 cudaStream_t stream, bool pdl) {
     switch (A) {
-        case 1: return launch_rt_seg_a<1>(a, smem, stream);
-        case 2: return launch_rt_seg_a<2>(a, smem, stream);
-        case 3: return launch_rt_seg_a<3>(a, smem, stream);
-        case 4: return launch_rt_seg_a<4>(a, smem, stream);
-        case 5: return launch_rt_seg_a<5>(a, smem, stream);
-        case 6: return launch_rt_seg_a<6>(a, smem, stream);
-        case 7: return launch_rt_seg_a<7>(a, smem, stream);
-        case 8: return launch_rt_seg_a<8>(a, smem, stream);
+        case 1: return launch_rt_seg_a<1>(m, a, smem, smem_optin, cache.configured[1], stream, pdl);
+        case 2: return launch_rt_seg_a<2>(m, a, smem, smem_optin, cache.configured[2], stream, pdl);
+        case 3: return launch_rt_seg_a<3>(m, a, smem, smem_optin, cache.configured[3], stream, pdl);
+        case 4: return launch_rt_seg_a<4>(m, a, smem, smem_optin, cache.configured[4], stream, pdl);
+        case 5: return launch_rt_seg_a<5>(m, a, smem, smem_optin, cache.configured[5], stream, pdl);
+        case 6: return launch_rt_seg_a<6>(m, a, smem, smem_optin, cache.configured[6], stream, pdl);
+        case 7: return launch_rt_seg_a<7>(m, a, smem, smem_optin, cache.configured[7], stream, pdl);
+        case 8: return launch_rt_seg_a<8>(m, a, smem, smem_optin, cache.configured[8], stream, pdl);
         default: return cudaErrorInvalidValue;
     }
 }

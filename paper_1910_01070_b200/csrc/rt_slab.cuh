@@ -106,15 +106,18 @@ __device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity
     }
 }
 // TMA: one box of the 4-D table view {nu, ip, iT, s} / the 3-D CIA view {nu, iT, c} -> shared memory
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
+// (dst: generic pointer to shared memory, or nullptr with the shared-memory byte address in dst_addr)
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3,
+                                            uint32_t dst_addr = 0) {
     asm volatile(
         "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+        ::"r"(dst ? smem_u32(dst) : dst_addr), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2,
+                                            uint32_t dst_addr = 0) {
     asm volatile(
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+        ::"r"(dst ? smem_u32(dst) : dst_addr), "l"((uint64_t)tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
 __device__ __forceinline__ void cp_async_16(uint32_t dst, const void* src) {
@@ -343,6 +346,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
     const bool model_valid = b < a.B;
     if (!model_valid) b = a.B - 1;           // still takes part in the slot hand-shake
     float* xw = xs_s + warp * a.x_floats;
+    pdl_wait();                    // records, x and flags come from the prep kernel (the producer streams static tables: no wait)
     for (int i = lane; i < a.x_floats; i += 32) xw[i] = a.model_x[(size_t)b * a.x_floats + i];
     __syncwarp();
 
@@ -489,6 +493,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
         }
     }
 
+    pdl_launch_dependents();
     if (!model_valid) return;
     float* out = a.flux + (size_t)b * a.flux_stride;       // written in grid order: columns of the padding map to >= nNu
     const bool one = gnu.x < a.nNu, two = gnu.y < a.nNu;
@@ -545,7 +550,7 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
 // size one context happens to need, so contexts with different table shapes cannot lower it for each other.
 template <int A, int NW, int MINB>
 inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
-                                    bool& configured, cudaStream_t stream) {
+                                    bool& configured, cudaStream_t stream, bool pdl) {
     const size_t smem = p.smem;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(k_rt_slab<A, NW, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_optin);
@@ -553,35 +558,34 @@ inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& t
         configured = true;
     }
     const dim3 grid((a.B + NW - 1) / NW, (a.nNu + kSlabTile - 1) / kSlabTile);
-    k_rt_slab<A, NW, MINB><<<grid, (NW + 1) * 32, smem, stream>>>(tms, tmc, a);
-    return cudaGetLastError();
+    return launch_kernel(k_rt_slab<A, NW, MINB>, grid, dim3((NW + 1) * 32), smem, stream, pdl, tms, tmc, a);
 }
 
 struct SlabSmemCache { bool configured[kMaxAngles + 1][4] = {}; };     // [A][models-per-CTA variant], one per context
 
 template <int A>
 inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
-                                    SlabSmemCache& cache, cudaStream_t stream) {
+                                    SlabSmemCache& cache, cudaStream_t stream, bool pdl) {
     switch (p.NW) {
-        case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p, cache.configured[A][0], stream);
-        case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p, cache.configured[A][1], stream);
-        case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p, cache.configured[A][2], stream);
-        case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p, cache.configured[A][3], stream);
+        case 8:  return launch_rt_slab_t<A, 8, 3>(tms, tmc, a, p, cache.configured[A][0], stream, pdl);
+        case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p, cache.configured[A][1], stream, pdl);
+        case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p, cache.configured[A][2], stream, pdl);
+        case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p, cache.configured[A][3], stream, pdl);
         default: return cudaErrorInvalidValue;
     }
 }
 
 inline cudaError_t launch_rt_slab(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
-                                  SlabSmemCache& cache, cudaStream_t stream) {
+                                  SlabSmemCache& cache, cudaStream_t stream, bool pdl) {
     switch (a.ang.n) {
-        case 1: return launch_rt_slab_a<1>(tms, tmc, a, p, cache, stream);
-        case 2: return launch_rt_slab_a<2>(tms, tmc, a, p, cache, stream);
-        case 3: return launch_rt_slab_a<3>(tms, tmc, a, p, cache, stream);
-        case 4: return launch_rt_slab_a<4>(tms, tmc, a, p, cache, stream);
-        case 5: return launch_rt_slab_a<5>(tms, tmc, a, p, cache, stream);
-        case 6: return launch_rt_slab_a<6>(tms, tmc, a, p, cache, stream);
-        case 7: return launch_rt_slab_a<7>(tms, tmc, a, p, cache, stream);
-        case 8: return launch_rt_slab_a<8>(tms, tmc, a, p, cache, stream);
+        case 1: return launch_rt_slab_a<1>(tms, tmc, a, p, cache, stream, pdl);
+        case 2: return launch_rt_slab_a<2>(tms, tmc, a, p, cache, stream, pdl);
+        case 3: return launch_rt_slab_a<3>(tms, tmc, a, p, cache, stream, pdl);
+        case 4: return launch_rt_slab_a<4>(tms, tmc, a, p, cache, stream, pdl);
+        case 5: return launch_rt_slab_a<5>(tms, tmc, a, p, cache, stream, pdl);
+        case 6: return launch_rt_slab_a<6>(tms, tmc, a, p, cache, stream, pdl);
+        case 7: return launch_rt_slab_a<7>(tms, tmc, a, p, cache, stream, pdl);
+        case 8: return launch_rt_slab_a<8>(tms, tmc, a, p, cache, stream, pdl);
         default: return cudaErrorInvalidValue;
     }
 }

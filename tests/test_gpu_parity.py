@@ -45,9 +45,11 @@ def wl3(torch_cuda):
     return W.make_workload(3, device=_gen_device(torch_cuda))
 
 
-def _run(torch, wl, params, kernel=0, highres=True, models_per_cta=0):
+def _run(torch, wl, params, kernel=0, highres=True, models_per_cta=0, nu_order=None):
     from paper_1910_01070_b200 import Helios
     h = Helios(0)
+    if nu_order is not None:
+        h.set_nu_order(nu_order)
     h.setup_workload(wl)
     h.set_kernel(kernel, models_per_cta)
     p = torch.as_tensor(np.ascontiguousarray(params), device="cuda:0")
@@ -487,21 +489,42 @@ def test_unphysical_models_are_rejected(torch_cuda, oracle, wl1, kernel):
 
 def test_small_batches_take_the_level_parallel_kernel_and_agree_with_the_staged_one(torch_cuda, oracle, wl2):
     """configs[2] tables with B = 1, 2, 4 in the launch configuration bench.py times for small batches
-    (kernel = auto -> level-parallel up to the measured crossover B = 4): every model against the oracle, and against
+    (kernel = auto -> level-parallel up to the measured crossover B = 8): every model against the oracle, and against
     the staged kernel's result for the same vectors (different operation order: agreement to a few ulp, not bitwise)."""
-    params = wl2.params[:8]
+    params = wl2.params[:16]
     ref = oracle.forward_workload(wl2, params=params, want_flux=True)
     spec_s, logl_s, flux_s, _ = _run(torch_cuda, wl2, params, kernel=2)
-    for B in (1, 2, 4, 8):
+    for B in (1, 2, 4, 8, 16):
         spec, logl, flux, _ = _run(torch_cuda, wl2, params[:B], kernel=0)
         assert _relerr(flux, ref["flux_hr"][:B]) <= TOL_FLUX
         assert _relerr(spec, ref["spectra"][:B]) <= TOL_FLUX
         _check_logl(wl2, logl, {"spectra": ref["spectra"][:B], "logl": ref["logl"][:B]}, spec)
         assert _relerr(flux, flux_s[:B]) <= 5e-6
-        forced = _run(torch_cuda, wl2, params[:B], kernel=3 if B <= 4 else 2)
+        forced = _run(torch_cuda, wl2, params[:B], kernel=3 if B <= 8 else 2)
         assert np.array_equal(forced[0], spec) and np.array_equal(forced[2], flux)     # which kernel auto really took
-    near = W.near_truth_params(wl2.cfg, 4)
+    near = W.near_truth_params(wl2.cfg, 12)[:8]     # the set of test_logl_near_truth_absolute_tolerance (DESIGN.md 'logL tolerance')
     refn = oracle.forward_workload(wl2, params=near)
     specn, logln, _, _ = _run(torch_cuda, wl2, near, kernel=0, highres=False)
     assert np.max(np.abs(logln - refn["logl"])) <= TOL_LOGL_ABS
-    _record("configs[2] near truth, B = 4 (level-parallel)", max_abs_dlogl=float(np.max(np.abs(logln - refn["logl"]))), n_models=4)
+    _record("configs[2] near truth, B = 8 (level-parallel)", max_abs_dlogl=float(np.max(np.abs(logln - refn["logl"]))), n_models=8)
+
+
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
+def test_wavenumber_order_tables_give_the_same_results(torch_cuda, oracle, wl1, kernel):
+    """HELIOS_OPT_NU_ORDER: the resident tables keep their columns in wavenumber order (0) or sorted by a reference
+    opacity (1, the default, which every other test runs).  Both against the oracle, and against each other: in the
+    direct kernel a wavenumber's arithmetic does not depend on its neighbours, so the two layouts agree bit for bit;
+    the staged and level-parallel kernels pick the thin / thick / general form of a layer's update per WARP, i.e.
+    depending on which 64 columns sit together, and those forms differ in the last bits."""
+    params = wl1.params[:24]
+    ref = oracle.forward_workload(wl1, params=params, want_flux=True)
+    out = {}
+    for order in (0, 1):
+        spec, logl, flux, _ = _run(torch_cuda, wl1, params, kernel=kernel, nu_order=order)
+        assert _relerr(flux, ref["flux_hr"]) <= TOL_FLUX and _relerr(spec, ref["spectra"]) <= TOL_FLUX
+        _check_logl(wl1, logl, ref, spec)
+        out[order] = (spec, logl, flux)
+    if kernel == 1:
+        assert np.array_equal(out[0][2], out[1][2]) and np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    else:
+        assert _relerr(out[0][2], out[1][2]) <= 5e-6 and _relerr(out[0][0], out[1][0]) <= 5e-6
