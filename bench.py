@@ -34,8 +34,8 @@ NOMINAL_FMA_PER_CLK_SM, NOMINAL_MUFU_PER_CLK_SM, NOMINAL_SM_MHZ = 128.0, 16.0, 1
 HBM_NOMINAL_GBS = 8000.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
 # ncu --set full captures summarised in profiles/ (None until captured for this workload).
-NCU_TRAFFIC_BYTES = {2: 216309248 + 16101120,       # profiles/r01_k_rt_slab_ncu_full.txt
-                     3: 1273274000 + 341796864}     # profiles/r01_k_rt_slab_cfg3_ncu_full.txt
+NCU_TRAFFIC_BYTES = {2: 220265984 + 8241152,        # profiles/r02_k_rt_slab_cfg2_ncu_full.txt
+                     3: 3726840000 + 2682859000}    # profiles/r02_k_rt_slab_cfg3_ncu_full.txt (flux: scattered 4-byte writes)
 
 
 def algorithmic_ops(cfg):
@@ -347,7 +347,10 @@ def run_gpu(args):
                    "kernel": {0: "auto", 1: "direct", 2: "slab", 3: "level-parallel"}[args.kernel]},
         "points_per_s": value * cfg.n_nu,
         "stage_ms_per_call": stage,
-        "roofline": {"bound": "alu", "kernel": "fused interpolate+tau+RT", "achieved": ach_tflops,
+        "roofline": {"bound": "alu", "kernel": "fused interpolate+tau+RT (k_rt_slab / k_rt_seg)", "achieved": ach_tflops,
+                     "achieved_is": "algorithmic FMAs of the method (4-tap bilinear per species and level) x 2 flop / kernel time: "
+                                    "useful work per second, not pipe utilisation (ncu pipe counters: profiles/r02_*)",
+                     "algorithmic_bytes": must_move_bytes(cfg, B_call),
                      "peak": alu_peak, "unit": "TFLOP/s", "frac": ach_tflops / alu_peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(cfg.index) if args.batch <= 0 and not teff else None,
                      "peak_source": peak_src, "peak_fma_per_clk_sm": fma_clk, "peak_sm_mhz": sm_mhz,
