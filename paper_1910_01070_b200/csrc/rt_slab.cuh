@@ -242,7 +242,7 @@ __device__ __forceinline__ void angle_step_w(float2& H, float2 dtau, float2 ndta
     const float2 w = make_float2(dtau.x < thr ? wn.x : wk.x, dtau.y < thr ? wn.y : wk.y);
     H = __ffma2_rn(w, __fadd2_rn(q, neg2(H)), H);
 }
-// angles K0 .. K1-1 with one kind of step: 0 general, 1 thick only, 2 thin only, 3 general in the w form
+// angles K0 .. K1-1 with one kind of step: 0 general, 1 thick only, 2 thin only, 3 general in the w form, 4 saturated
 template <int A, int K0, int K1, int MODE>
 __device__ __forceinline__ void angle_range(float2 (&H)[A], float2 dtau, float2 ndtau, float2 q, float2 dS) {
     if constexpr (K0 < K1) {
@@ -250,6 +250,7 @@ __device__ __forceinline__ void angle_range(float2 (&H)[A], float2 dtau, float2 
         if constexpr (MODE == 1) angle_step_thick<A, K0>(H[K0], ndtau, q);
         if constexpr (MODE == 2) angle_step_thin<A, K0>(H[K0], dtau, ndtau, dS);
         if constexpr (MODE == 3) angle_step_w<A, K0>(H[K0], dtau, ndtau, q);
+        if constexpr (MODE == 4) H[K0] = __ffma2_rn(make_float2(0.0f, 0.0f), H[K0], q);    // = q, updated in place like the other forms
         angle_range<A, K0 + 1, K1, MODE>(H, dtau, ndtau, q, dS);
     }
 }
@@ -269,10 +270,17 @@ __device__ __forceinline__ float2 flux_sum(const float2 (&H)[A], float2 S_top, s
 //   all-thin   every lane has dtau < 0.25 mu_0        -> only the polynomial branch, for every angle
 //   all-thick  every lane has dtau >= 0.25 mu_{A-1}   -> only the ex2 branch, for every angle
 // dtau >= 0, so the order of the floats is the order of their bit patterns (REDUX works on integers).
+//   saturated  every lane has e^{-dtau/mu_k} < 2^-30 for the n smallest mu_k  -> H_k = e H_k + (1 - e) q = q for those
+//              (deep layers: 44 % of the all-thick (warp, layer) pairs at configs[3] are saturated in all 8 angles)
 template <int A>
 struct LayerLimits {
     static constexpr unsigned all_thick = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][A - 1]));
     static constexpr unsigned all_thin = __builtin_bit_cast(unsigned, (float)(0.25 * kGLmu[A - 1][0]));
+    // dtau above which the n smallest-mu angles are saturated (30 ln 2 = 20.794); n = A, 4, 2, 1
+    static constexpr unsigned sat_all = __builtin_bit_cast(unsigned, (float)(20.7944154168 * kGLmu[A - 1][A - 1]));
+    static constexpr unsigned sat4 = __builtin_bit_cast(unsigned, (float)(20.7944154168 * kGLmu[A - 1][A >= 4 ? 3 : 0]));
+    static constexpr unsigned sat2 = __builtin_bit_cast(unsigned, (float)(20.7944154168 * kGLmu[A - 1][A >= 2 ? 1 : 0]));
+    static constexpr unsigned sat1 = __builtin_bit_cast(unsigned, (float)(20.7944154168 * kGLmu[A - 1][0]));
 };
 
 // Level records are staged per warp: blocks of kRecBlk levels, double-buffered, copied with cp.async one block ahead
@@ -458,7 +466,18 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
                 } else {
                     const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
                     if (d_lo >= LayerLimits<A>::all_thick) {
-                        all_angles_thick<A>(H, ndtau, q, std::make_integer_sequence<int, A>{});
+                        constexpr int N4 = A >= 8 ? 4 : 0, N1 = A >= 4 ? 1 : 0;
+                        if (d_lo >= LayerLimits<A>::sat_all) {
+                            angle_range<A, 0, A, 4>(H, dtau, ndtau, q, dS);
+                        } else if (N4 > 0 && d_lo >= LayerLimits<A>::sat4) {
+                            angle_range<A, 0, N4, 4>(H, dtau, ndtau, q, dS);
+                            angle_range<A, N4, A, 1>(H, dtau, ndtau, q, dS);
+                        } else if (N1 > 0 && d_lo >= LayerLimits<A>::sat1) {
+                            angle_range<A, 0, N1, 4>(H, dtau, ndtau, q, dS);
+                            angle_range<A, N1, A, 1>(H, dtau, ndtau, q, dS);
+                        } else {
+                            all_angles_thick<A>(H, ndtau, q, std::make_integer_sequence<int, A>{});
+                        }
                     } else {
                         constexpr int GM = 3;
                         const float2 dtc = make_float2(fmaxf(dtau.x, 1e-20f), fmaxf(dtau.y, 1e-20f));
