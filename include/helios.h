@@ -71,8 +71,10 @@ int  helios_set_stream(helios_ctx* ctx, void* cuda_stream);
 const char* helios_last_error(const helios_ctx* ctx);
 int  helios_set_option(helios_ctx* ctx, int key, int value);
 
-/* Opacity tables.  Copies everything to HBM as fp32,
- * nu-contiguous, rows padded to 256 B (64 floats, the staged kernel's tile).
+/* Opacity tables.  Copies everything to HBM as fp32, one wavenumber per column,
+ * rows padded to 256 B (64 floats, the kernels' tile).  The columns are kept in the order HELIOS_OPT_NU_ORDER
+ * selects (default: sorted by a reference opacity; the library maps column <-> wavenumber itself, every result
+ * is in wavenumber order).  Host tables are staged through one device buffer of nT*nP*nNu floats.
  *   T_grid_K        HOST [nT]  strictly increasing, arbitrary spacing (nT >= 2)
  *   log10p_grid_bar HOST [nP]  strictly increasing, arbitrary spacing (nP >= 2)
  *   wavenumber grid nu_i = nu0_cm1 + i*dnu_cm1, i < nNu (uniform, dnu > 0)

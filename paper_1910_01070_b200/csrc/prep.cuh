@@ -43,6 +43,8 @@ constexpr int kMaxTpNodes = 5;    // order <= 4
 constexpr int kPrepThreads = 128;
 constexpr int kPrepMaxSpecies = 64;
 constexpr int kPrepMaxLevels = 4096;
+constexpr int kPrepMaxTgrid = 256;
+constexpr int kPrepIpLevels = 1024;
 
 // Eq. 12: T(level) = sum_i T_dof[k q + i] l_i(xi).  In the ratio form the nodal temperatures are the
 // running products T_1 b_2 ... b_j (R28), rebuilt here for the element's q + 1 nodes.
@@ -65,8 +67,17 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
     __shared__ int s_ok;
     __shared__ short s_cell[kPrepMaxLevels];   // temperature cell of every level (cell-walk schedule below)
     __shared__ double s_T[kPrepMaxLevels];     // temperature of every level (each one is needed by three levels)
+    __shared__ short s_ip[kPrepIpLevels];      // pressure cell of every level (global memory for longer atmospheres)
+    __shared__ double s_Tg[kPrepMaxTgrid];     // the table's temperature grid (global memory when it is longer)
     const int b = blockIdx.x, tid = threadIdx.x;
     pdl_launch_dependents();       // the RT kernel may be scheduled now; it waits for this grid before reading the records
+    // static per-level data first, all loads in flight at once: with one model the kernel is a chain of dependent
+    // load latencies (the bisection on the temperature grid alone was five round trips to L2)
+    const double* Tg = a.nT <= kPrepMaxTgrid ? s_Tg : a.T_grid;
+    if (a.nT <= kPrepMaxTgrid) for (int k = tid; k < a.nT; k += kPrepThreads) s_Tg[k] = a.T_grid[k];
+    const bool ip_s = a.L <= kPrepIpLevels;
+    if (ip_s) for (int l = tid; l < a.L; l += kPrepThreads) s_ip[l] = (short)a.lvl_ip[l];
+    auto ip_of = [&](int l) { return ip_s ? (int)s_ip[l] : a.lvl_ip[l]; };
     const double* th = a.params + (size_t)b * a.P;
     const double* tpar = th + 2;
     const double* lvmr = th + 2 + a.NT;
@@ -142,9 +153,9 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
         int iT = 0;
         for (int hi = a.nT - 1; hi - iT > 1;) {       // bisection: T_grid[iT] <= T < T_grid[hi] (or T outside the grid)
             const int mid = (iT + hi) >> 1;
-            if (a.T_grid[mid] <= T) iT = mid; else hi = mid;
+            if (Tg[mid] <= T) iT = mid; else hi = mid;
         }
-        double t = (T - a.T_grid[iT]) / (a.T_grid[iT + 1] - a.T_grid[iT]);
+        double t = (T - Tg[iT]) / (Tg[iT + 1] - Tg[iT]);
         int clamped = a.lvl_pclamp[l];
         if (t < 0.0) { t = 0.0; clamped = 1; }
         if (t > 1.0) { t = 1.0; clamped = 1; }
@@ -188,7 +199,7 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
             }
             rec[o++] = pa_hi; rec[o++] = pa_lo;
             rec[o++] = (float)hdz_up;
-            rec[o++] = __int_as_float(iT * a.nP + a.lvl_ip[l]);
+            rec[o++] = __int_as_float(iT * a.nP + ip_of(l));
             rec[o++] = __int_as_float(iT);
             rec[o++] = (float)dtc_up;
         } else {                 // kSlabRecFloats floats, layout in common.cuh
@@ -215,12 +226,12 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
         for (int l = tid; l < a.L; l += kPrepThreads) {
             int kind = 0;
             if (l > 0) {
-                const int iT0 = s_cell[l - 1], ip0 = a.lvl_ip[l - 1], iT1 = s_cell[l], ip1 = a.lvl_ip[l];
+                const int iT0 = s_cell[l - 1], ip0 = ip_of(l - 1), iT1 = s_cell[l], ip1 = ip_of(l);
                 kind = ip1 == ip0 ? (iT1 == iT0 ? 4 : (iT1 == iT0 - 1 ? 1 : (iT1 == iT0 + 1 ? 2 : 0)))
                                   : ((iT1 == iT0 && ip1 == ip0 - 1) ? 3 : 0);
             }
             int j = l + 1;
-            while (j < a.L && s_cell[j] == s_cell[l] && a.lvl_ip[j] == a.lvl_ip[l]) ++j;
+            while (j < a.L && s_cell[j] == s_cell[l] && ip_of(j) == ip_of(l)) ++j;
             const int dist = j < a.L ? j - l : 0;
             a.rec[((size_t)b * a.L + l) * a.rec_floats + 11] = __int_as_float(kind | (dist << 8));
         }
