@@ -50,6 +50,11 @@ enum {
                                       sorted by a reference opacity, so that the 64 columns a warp owns are optically alike and
                                       take the kernels' warp-uniform thin / thick shortcuts; 0 = wavenumber order.  Results are
                                       always returned in wavenumber order. */
+#define HELIOS_OPT_FUSED_OBS   5   /* 1 = helios_forward_batch / helios_loglike_batch apply the instrument profile and the binning in
+                                      the epilogue of the RT kernel (bitwise-reproducible 64-bit integer atomics into M[b][j]) and never
+                                      write a high-resolution flux: no B x nNu buffer traffic, but the atomics cost more time than the
+                                      second kernel they replace (configs[3]: +2.1 ms of 44.5).  0 (default) = the
+                                      RT kernel writes the flux, k_obs_apply applies the operator. */
 #define HELIOS_OPT_TIMING      3   /* 1 = bracket every stage of the next calls with CUDA events on the context's stream */
 
 typedef struct helios_stats {

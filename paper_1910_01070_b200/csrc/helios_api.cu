@@ -71,6 +71,8 @@ struct helios_ctx {
     double* d_edges = nullptr; double* d_obs = nullptr; double* d_inv2var = nullptr; double* d_var = nullptr;
     double* d_addvar = nullptr;         // [cap_B] 10^epsilon per model
     int* d_row_ptr = nullptr; int* d_row_lo = nullptr; float* d_W = nullptr;
+    int* d_wt_ptr = nullptr; int* d_wt_j = nullptr; float* d_wt_w = nullptr;      // transposed operator (fused observation)
+    unsigned long long* d_acc = nullptr; float* d_q = nullptr;                     // [cap_B][J] integer sums and their scales
 
     // ---- workspace (grown on demand)
     int cap_B = 0;
@@ -82,7 +84,7 @@ struct helios_ctx {
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
     // ---- options / statistics
-    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0, opt_nu_order = 1;
+    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0, opt_nu_order = 1, opt_fused = 0;
     static constexpr int kTimingRing = 64;
     cudaEvent_t ev[kTimingRing][4] = {};
     bool ev_has_obs[kTimingRing] = {};
@@ -130,6 +132,7 @@ static void free_all(helios_ctx* c) {
     dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
     dfree(c->d_seg); dfree(c->d_load_ip);
     dfree(c->d_edges); dfree(c->d_obs); dfree(c->d_inv2var); dfree(c->d_var); dfree(c->d_addvar); dfree(c->d_row_ptr); dfree(c->d_row_lo); dfree(c->d_W);
+    dfree(c->d_wt_ptr); dfree(c->d_wt_j); dfree(c->d_wt_w); dfree(c->d_acc); dfree(c->d_q);
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x); dfree(c->d_counters);
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage);
@@ -359,6 +362,8 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24)
                 return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16, 20 or 24");
             c->opt_models_per_cta = value; return HELIOS_OK;
+        case HELIOS_OPT_FUSED_OBS:
+            c->opt_fused = value ? 1 : 0; return HELIOS_OK;
         case HELIOS_OPT_NU_ORDER:
             if (value != 0 && value != 1) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_NU_ORDER must be 0 (grid order) or 1 (opacity order)");
             c->opt_nu_order = value; return HELIOS_OK;
@@ -654,6 +659,27 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
     c->n_launches += 2;
     CU_TRY(c, cudaGetLastError());
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    {   // the operator by grid point (CSR, zeros dropped) for the fused epilogue of the RT kernels (obs.cuh); marshalling only
+        std::vector<float> Wh((size_t)row_ptr[J]);
+        CU_TRY(c, cudaMemcpy(Wh.data(), c->d_W, sizeof(float) * Wh.size(), cudaMemcpyDeviceToHost));
+        std::vector<int> wt_ptr(c->nNu + 1, 0), wt_j;
+        std::vector<float> wt_w;
+        for (int j = 0; j < J; ++j)
+            for (int e2 = row_ptr[j]; e2 < row_ptr[j + 1]; ++e2)
+                if (Wh[e2] != 0.0f) wt_ptr[row_lo[j] + (e2 - row_ptr[j]) + 1]++;
+        for (int i = 0; i < c->nNu; ++i) wt_ptr[i + 1] += wt_ptr[i];
+        wt_j.resize(wt_ptr[c->nNu]); wt_w.resize(wt_ptr[c->nNu]);
+        std::vector<int> fill(wt_ptr.begin(), wt_ptr.end() - 1);
+        for (int j = 0; j < J; ++j)
+            for (int e2 = row_ptr[j]; e2 < row_ptr[j + 1]; ++e2)
+                if (Wh[e2] != 0.0f) {
+                    const int i = row_lo[j] + (e2 - row_ptr[j]);
+                    wt_j[fill[i]] = j; wt_w[fill[i]] = Wh[e2]; fill[i]++;
+                }
+        CU_TRY(c, upload(c->d_wt_ptr, wt_ptr, c->stream));
+        CU_TRY(c, upload(c->d_wt_j, wt_j, c->stream));
+        CU_TRY(c, upload(c->d_wt_w, wt_w, c->stream));
+    }
 
     if (obs) {
         std::vector<double> o(obs, obs + J), i2v(J);
@@ -709,6 +735,7 @@ int helios_reserve(helios_ctx* c, int B) {
     dfree(c->d_rec); dfree(c->d_flux); dfree(c->d_scale); dfree(c->d_flag); dfree(c->d_model_x);
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage); dfree(c->d_addvar);
+    dfree(c->d_acc); dfree(c->d_q);
     c->cap_B = 0;
     const int rf = std::max(direct_rec_floats(c->S, c->C), kSlabRecFloats);
     c->flux_stride = c->stride;
@@ -727,6 +754,8 @@ int helios_reserve(helios_ctx* c, int B) {
     CU_TRY(c, cudaMalloc(&c->d_addvar, sizeof(double) * B));
     CU_TRY(c, cudaMalloc(&c->d_spectra_stage, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
     CU_TRY(c, cudaMalloc(&c->d_logl_stage, sizeof(double) * B));
+    CU_TRY(c, cudaMalloc(&c->d_acc, sizeof(unsigned long long) * (size_t)B * (c->J > 0 ? c->J : 1)));
+    CU_TRY(c, cudaMalloc(&c->d_q, sizeof(float) * (size_t)B * (c->J > 0 ? c->J : 1)));
     c->cap_B = B;
     return HELIOS_OK;
 }
@@ -736,7 +765,10 @@ static inline void stamp(helios_ctx* c, int which) {
 }
 
 // steps 0-4: params -> flux (DEVICE [B][flux_stride])
-static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride, int unit_scale = 0) {
+// fused: in/out -- on entry, the caller wants the observation operator applied in the RT kernel's epilogue (obs.cuh);
+// on return, whether the kernel that ran did (the direct fallback kernel does not, it writes the flux)
+static int run_flux(helios_ctx* c, int B, const double* params, float* flux, long long flux_stride, int unit_scale = 0,
+                    bool* fused = nullptr) {
     const SlabPlan plan = plan_slab(c, B);
     if (c->opt_kernel == 2 && !plan.ok)
         return fail(c, HELIOS_EINVAL, "staged kernel requested but unavailable for this table shape (shared memory / TMA)");
@@ -757,6 +789,14 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
     pa.rec = c->d_rec; pa.rec_floats = rf; pa.slab_layout = slab; pa.model_scale = c->d_scale; pa.model_flag = c->d_flag;
     pa.model_x = c->d_model_x; pa.x_floats = slab_x_floats(c->S, c->C);
     pa.counters = c->d_counters;
+    const bool fuse = fused && *fused && slab && c->have_obs;
+    if (fused) *fused = fuse;
+    FusedObs fo{};
+    if (fuse) {
+        fo.acc = c->d_acc; fo.q = c->d_q; fo.wt_ptr = c->d_wt_ptr; fo.wt_j = c->d_wt_j; fo.wt_w = c->d_wt_w; fo.J = c->J;
+        pa.fused_acc = c->d_acc; pa.fused_q = c->d_q; pa.J = c->J; pa.row_ptr = c->d_row_ptr; pa.row_lo = c->d_row_lo;
+        pa.nu0 = c->nu0; pa.dnu = c->dnu;
+    }
     // programmatic dependent launch of the RT and observation kernels (common.cuh); not with stage timing, whose
     // events between the kernels serialise them
     const bool pdl = !c->opt_timing;
@@ -771,7 +811,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         ga.sigma = c->d_sigma; ga.cia = c->d_cia; ga.stride = c->stride; ga.S = c->S; ga.C = c->C; ga.nT = c->nT; ga.nP = c->nP;
         ga.nNu = c->nNu; ga.L = c->L; ga.B = B; ga.rec = c->d_rec; ga.model_x = c->d_model_x; ga.x_floats = pa.x_floats;
         ga.model_scale = c->d_scale; ga.model_flag = c->d_flag; ga.lvl_ip = c->d_lvl_ip; ga.nu_index = c->d_nu_index; ga.nu0 = c->nu0; ga.dnu = c->dnu;
-        ga.flux = flux; ga.flux_stride = flux_stride; ga.n_chunks = seg.n_chunks; ga.chunk_len = seg.chunk_len;
+        ga.flux = flux; ga.flux_stride = flux_stride; ga.fused = fo; ga.n_chunks = seg.n_chunks; ga.chunk_len = seg.chunk_len;
         cudaError_t e = launch_rt_seg(c->A, c->seg_maps, ga, seg.smem, c->smem_optin, c->seg_smem, c->stream, pdl);
         if (e != cudaSuccess) return fail(c, HELIOS_ECUDA, "level-parallel kernel launch failed: %s", cudaGetErrorString(e));
         c->n_launches += 1;
@@ -783,7 +823,7 @@ static int run_flux(helios_ctx* c, int B, const double* params, float* flux, lon
         sa.S = c->S; sa.C = c->C; sa.nT = c->nT; sa.nNu = c->nNu; sa.L = c->L; sa.B = B;
         sa.rec = c->d_rec; sa.model_x = c->d_model_x; sa.x_floats = pa.x_floats;
         sa.model_scale = c->d_scale; sa.model_flag = c->d_flag; sa.nu0 = c->nu0; sa.dnu = c->dnu; sa.nu_index = c->d_nu_index;
-        sa.flux = flux; sa.flux_stride = flux_stride;
+        sa.flux = flux; sa.flux_stride = flux_stride; sa.fused = fo;
         sa.seg = c->d_seg + (size_t)(plan.ring - 1) * c->n_seg; sa.load_ip = c->d_load_ip;
         sa.n_seg = c->n_seg; sa.n_loads = c->n_loads; sa.ring = plan.ring; sa.ang = c->ang;
         cudaError_t e = launch_rt_slab(c->tm_sigma, c->tm_cia, sa, plan, c->slab_smem, c->stream, pdl);
@@ -850,7 +890,8 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     CU_TRY(c, cudaSetDevice(c->device));
     if ((rc = helios_reserve(c, B))) return rc;
     c->n_models += B;
-    if ((rc = run_flux(c, B, params, c->d_flux, c->flux_stride))) return rc;
+    bool fused = c->opt_fused != 0;
+    if ((rc = run_flux(c, B, params, c->d_flux, c->flux_stride, 0, &fused))) return rc;
     ObsApplyArgs oa{};
     oa.J = c->J; oa.row_ptr = c->d_row_ptr; oa.row_lo = c->d_row_lo; oa.W = c->d_W; oa.flux = c->d_flux;
     oa.flux_stride = c->flux_stride; oa.model_flag = c->d_flag; oa.obs = c->d_obs; oa.inv2var = c->d_inv2var;
@@ -860,7 +901,10 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     // one bin per warp while 64-bin CTAs would leave SMs idle (the choice depends on B only through this threshold;
     // kObsSmallBatchCtas is fixed, so a given (B, J) always takes the same variant)
     const bool pdl = !c->opt_timing;
-    if ((long long)B * ((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta) < kObsSmallBatchCtas)
+    if (fused) {
+        FusedObs fo{c->d_acc, c->d_q, c->d_wt_ptr, c->d_wt_j, c->d_wt_w, c->J};
+        CU_TRY(c, launch_kernel(k_obs_final, dim3(B), dim3(kObsThreads), 0, c->stream, pdl, oa, fo));
+    } else if ((long long)B * ((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta) < kObsSmallBatchCtas)
         CU_TRY(c, launch_kernel(k_obs_apply<1>, dim3((c->J + 7) / 8, B), dim3(kObsThreads), 0, c->stream, pdl, oa));
     else
         CU_TRY(c, launch_kernel(k_obs_apply<8>, dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), dim3(kObsThreads), 0,

@@ -11,6 +11,8 @@
 //          (= the weight of F_d[k] in the bin mean of the piecewise-linear interpolant).
 // DESIGN.md R15, R17, R18.
 #pragma once
+#include <math_constants.h>
+
 #include "common.cuh"
 
 namespace helios {
@@ -188,6 +190,98 @@ __global__ void __launch_bounds__(kObsThreads) k_obs_apply(ObsApplyArgs a) {
         a.logl[b] = bad ? -CUDART_INF : (a.addvar ? -tree[0] : a.logl_const - tree[0]);
         a.arrived[b] = 0;
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// Fused variant: the RT kernels apply the operator themselves, in their epilogue, and no high-resolution flux
+// is written at all (north_star: "writes only logL when spectra are not requested").  A lane that has just
+// finished the flux F of grid point i adds W_ji F to M_j for the handful of bins j whose band holds i
+// (the transposed operator, CSR by grid point: wt_ptr / wt_j / wt_w).  The wavenumbers of a warp are
+// scattered over the grid (opacity order) and a bin is fed by ~1500 CTAs, so the sums are ATOMIC -- and to keep
+// them bitwise reproducible they are INTEGER: every term is scaled by a per-(model, bin) power of two q_bj,
+// rounded to a 64-bit integer and added with a 64-bit atomic; integer addition is associative, so the result does
+// not depend on the order in which the CTAs arrive.  q_bj = 2^(60 - e) with 2^e > the largest value M_j can take
+// for that model, pi f (R/d)^2 max over the band of B_nu(T_max) (every intensity is a convex combination of level
+// sources, W rows are non-negative and sum to 1), worked out by k_prep: the sum cannot overflow, and one unit is
+// 2^-60 of that bound.  k_obs_final turns the integers back into M_j (exactly, in fp64) and forms chi-square with
+// the same grouping and tree as k_obs_apply.
+// ---------------------------------------------------------------------------------------
+struct FusedObs {
+    unsigned long long* acc;   // DEVICE [B][J]  integer sums, zeroed by k_prep; nullptr = not fused (write the flux)
+    const float* q;            // DEVICE [B][J]  power-of-two scales (0: model rejected or flux identically 0)
+    const int* wt_ptr;         // DEVICE [nNu + 1]
+    const int* wt_j;           // DEVICE [nnz]  bin
+    const float* wt_w;         // DEVICE [nnz]  W_ji (zeros dropped)
+    int J;
+};
+
+__device__ __forceinline__ void fused_accumulate(const FusedObs& f, int b, int i, float F) {
+    const int t0 = __ldg(f.wt_ptr + i), t1 = __ldg(f.wt_ptr + i + 1);
+    unsigned long long* acc = f.acc + (size_t)b * f.J;
+    const float* q = f.q + (size_t)b * f.J;
+    for (int t = t0; t < t1; ++t) {
+        const int j = __ldg(f.wt_j + t);
+        const float v = __fmul_rn(__fmul_rn(__ldg(f.wt_w + t), F), __ldg(q + j));       // the scale is a power of two: exact
+        atomicAdd(acc + j, (unsigned long long)__float2ll_rn(v));
+    }
+}
+
+// B_nu(T) at its maximum over [nu_a, nu_b] (the Planck function is unimodal; peak at c2 nu / T = 2.821439...), fp64
+__device__ __forceinline__ double planck_band_max(double nu_a, double nu_b, double T) {
+    double nu = 2.8214393721220787 * T / kC2;
+    nu = fmin(fmax(nu, nu_a), nu_b);
+    return kC1 * nu * nu * nu / expm1(kC2 * nu / T);
+}
+// q_bj for one (model, bin): bound = largest possible M_j; returns 2^(60 - e), bound < 2^e, clamped to the fp32 range
+__device__ __forceinline__ float fused_scale(double bound) {
+    if (!(bound > 0.0) || !isfinite(bound)) return 0.0f;
+    int e;
+    frexp(bound, &e);                     // bound = m 2^e, 0.5 <= m < 1
+    int qe = 60 - e;
+    qe = qe > 127 ? 127 : (qe < -126 ? -126 : qe);
+    return __int_as_float((qe + 127) << 23);
+}
+
+__global__ void __launch_bounds__(kObsThreads) k_obs_final(ObsApplyArgs a, FusedObs f) {
+    __shared__ double tree[kObsThreads];
+    const int b = blockIdx.x;
+    pdl_wait();                    // the integer sums (RT kernel), scales and flags (prep kernel) are complete
+    const bool bad = a.model_flag[b] != 0;
+    const unsigned long long* acc = f.acc + (size_t)b * a.J;
+    const float* q = f.q + (size_t)b * a.J;
+    const double add = a.addvar ? a.addvar[b] : 0.0;
+    const int n_groups = (a.J + 7) / 8;
+    double t = 0.0;
+    for (int g = threadIdx.x; g < n_groups; g += kObsThreads) {       // thread t: groups t, t + 256, ... (k_obs_apply's order)
+        double chi2 = 0.0;
+        for (int j = 8 * g; j < min(8 * g + 8, a.J); ++j) {
+            const float qj = q[j];
+            float M = qj > 0.0f ? (float)((double)(long long)acc[j] * (1.0 / (double)qj)) : 0.0f;
+            if (bad) M = __int_as_float(0x7fc00000);
+            if (a.spectra) a.spectra[(size_t)b * a.J + j] = M;
+            if (a.logl) {
+                const double r = a.obs[j] - (double)M;
+                double term;
+                if (a.addvar) {                       // Eq. 23
+                    const double s2 = a.var[j] + add;
+                    term = __dadd_rn(__ddiv_rn(__dmul_rn(r, r), __dmul_rn(2.0, s2)), __dmul_rn(0.5, log(__dmul_rn(2.0 * kPi, s2))));
+                } else {
+                    term = __dmul_rn(__dmul_rn(r, r), a.inv2var[j]);
+                }
+                chi2 = __dadd_rn(chi2, term);
+            }
+        }
+        t += chi2;
+    }
+    if (!a.logl) return;
+    tree[threadIdx.x] = t;
+    __syncthreads();
+#pragma unroll
+    for (int o = kObsThreads / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) tree[threadIdx.x] += tree[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) a.logl[b] = bad ? -CUDART_INF : (a.addvar ? -tree[0] : a.logl_const - tree[0]);
 }
 
 // ---------------------------------------------------------------------------------------

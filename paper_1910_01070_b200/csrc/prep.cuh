@@ -8,6 +8,7 @@
 // (model, level) repeated ~S+3 double-precision pow() calls in every thread: 20 us for one model.)
 #pragma once
 #include "common.cuh"
+#include "obs.cuh"
 
 namespace helios {
 
@@ -37,6 +38,13 @@ struct PrepArgs {
     float* model_scale;       // DEVICE [B]  f * flux_const * 2 pi
     int*   model_flag;        // DEVICE [B]  1 = rejected model
     unsigned long long* counters;  // [0] clamped pairs, [1] rejected models
+    // fused observation (obs.cuh): per (model, bin) the integer accumulator is zeroed and its power-of-two scale set
+    unsigned long long* fused_acc; // DEVICE [B][J] or nullptr
+    float* fused_q;                // DEVICE [B][J]
+    int J;
+    const int* row_ptr;            // DEVICE [J + 1]  band of every bin: grid points row_lo[j] .. row_lo[j] + len_j - 1
+    const int* row_lo;             // DEVICE [J]
+    double nu0, dnu;
 };
 
 constexpr int kMaxTpNodes = 5;    // order <= 4
@@ -234,6 +242,28 @@ __global__ void __launch_bounds__(kPrepThreads) k_prep(PrepArgs a) {
             while (j < a.L && s_cell[j] == s_cell[l] && ip_of(j) == ip_of(l)) ++j;
             const int dist = j < a.L ? j - l : 0;
             a.rec[((size_t)b * a.L + l) * a.rec_floats + 11] = __int_as_float(kind | (dist << 8));
+        }
+    }
+    if (a.fused_acc) {
+        // the largest value a bin can take for this model: pi f (R/d)^2 max_band B_nu(T_max) (see obs.cuh)
+        __shared__ double s_red[kPrepThreads];
+        double tmax = 0.0;
+        for (int l = tid; l < a.L; l += kPrepThreads) tmax = fmax(tmax, s_T[l]);
+        s_red[tid] = tmax;
+        __syncthreads();
+        for (int o = kPrepThreads / 2; o > 0; o >>= 1) {
+            if (tid < o) s_red[tid] = fmax(s_red[tid], s_red[tid + o]);
+            __syncthreads();
+        }
+        tmax = s_red[0];
+        const bool ok = model_ok && !any_bad;
+        const double amp = 0.5 * sm[6] * 2.0 * kPi;             // model_scale (below) x sum_k w_k mu_k
+        for (int j = tid; j < a.J; j += kPrepThreads) {
+            const int lo = a.row_lo[j], len = a.row_ptr[j + 1] - a.row_ptr[j];
+            float q = 0.0f;
+            if (ok && len > 0) q = fused_scale(amp * planck_band_max(a.nu0 + a.dnu * lo, a.nu0 + a.dnu * (lo + len - 1), tmax));
+            a.fused_q[(size_t)b * a.J + j] = q;
+            a.fused_acc[(size_t)b * a.J + j] = 0ull;
         }
     }
     if (tid == 0) {

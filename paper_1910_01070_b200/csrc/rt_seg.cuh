@@ -46,8 +46,9 @@ struct SegArgs {
     const int* lvl_ip;        // DEVICE [L] pressure cell of each level
     const int* nu_index;      // DEVICE [stride]  wavenumber grid index of every table column (helios_load_opacity)
     double nu0, dnu;
-    float* flux;              // DEVICE [B][flux_stride]
+    float* flux;              // DEVICE [B][flux_stride]  (not written when fused.acc != nullptr)
     long long flux_stride;
+    FusedObs fused;           // observation operator applied in the epilogue (obs.cuh)
     int n_chunks, chunk_len;  // chunk c owns the layers 1 + c len .. min(L - 1, (c + 1) len)  (layer j: levels j-1, j)
 };
 
@@ -296,17 +297,19 @@ k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUte
             H[k] = __ffma2_rn(psi, H[k], cc);
         }
     }
-    float* out = a.flux + (size_t)b * a.flux_stride;
     const bool one = gnu.x < a.nNu, two = gnu.y < a.nNu;
-    if (a.model_flag[b]) {
-        if (one) out[gnu.x] = __int_as_float(0x7fc00000);
-        if (two) out[gnu.y] = __int_as_float(0x7fc00000);
-        return;
-    }
+    const bool rejected = a.model_flag[b] != 0;
     const float2 acc = flux_sum<A>(H, reinterpret_cast<const float2*>(stop)[lane], std::make_integer_sequence<int, A>{});
     const float scale = a.model_scale[b];
-    if (one) out[gnu.x] = scale * acc.x;
-    if (two) out[gnu.y] = scale * acc.y;
+    if (a.fused.acc) {               // convolve + bin here: integer atomics into M[b][j] (obs.cuh); no flux is written
+        if (rejected) return;
+        if (one) fused_accumulate(a.fused, b, gnu.x, scale * acc.x);
+        if (two) fused_accumulate(a.fused, b, gnu.y, scale * acc.y);
+        return;
+    }
+    float* out = a.flux + (size_t)b * a.flux_stride;
+    if (one) out[gnu.x] = rejected ? __int_as_float(0x7fc00000) : scale * acc.x;
+    if (two) out[gnu.y] = rejected ? __int_as_float(0x7fc00000) : scale * acc.y;
 }
 
 struct SegPlan {

@@ -32,6 +32,7 @@
 #include <utility>
 
 #include "common.cuh"
+#include "obs.cuh"
 
 namespace helios {
 
@@ -58,8 +59,9 @@ struct SlabArgs {
     const int* model_flag;
     double nu0, dnu;
     const int* nu_index;            // DEVICE [stride]  wavenumber grid index of every table column (helios_load_opacity)
-    float* flux;                    // DEVICE [B][flux_stride]
+    float* flux;                    // DEVICE [B][flux_stride]  (not written when fused.acc != nullptr)
     long long flux_stride;
+    FusedObs fused;                 // observation operator applied in the epilogue (obs.cuh)
     // plane schedule (helios_set_atmosphere), resolved for this launch's ring depth
     const SlabSeg* seg;             // DEVICE [n_seg]
     const int* load_ip;             // DEVICE [n_loads] pressure node of each load, in issue order
@@ -514,18 +516,20 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
 
     pdl_launch_dependents();
     if (!model_valid) return;
-    float* out = a.flux + (size_t)b * a.flux_stride;       // written in grid order: columns of the padding map to >= nNu
     const bool one = gnu.x < a.nNu, two = gnu.y < a.nNu;
-    if (a.model_flag[b]) {
-        if (one) out[gnu.x] = __int_as_float(0x7fc00000);
-        if (two) out[gnu.y] = __int_as_float(0x7fc00000);
-        return;
-    }
+    const bool rejected = a.model_flag[b] != 0;
     // F+ = 2 pi sum_k w_k mu_k I_k (Eq. 8), I_k = mu_k H_k + S_top;  F = f (R/d)^2 F+ (Eq. 9)
     const float2 acc = flux_sum<A>(H, S_prev, std::make_integer_sequence<int, A>{});
     const float scale = a.model_scale[b];
-    if (one) out[gnu.x] = scale * acc.x;
-    if (two) out[gnu.y] = scale * acc.y;
+    if (a.fused.acc) {               // convolve + bin here: integer atomics into M[b][j] (obs.cuh); no flux is written
+        if (rejected) return;
+        if (one) fused_accumulate(a.fused, b, gnu.x, scale * acc.x);
+        if (two) fused_accumulate(a.fused, b, gnu.y, scale * acc.y);
+        return;
+    }
+    float* out = a.flux + (size_t)b * a.flux_stride;       // written in grid order: columns of the padding map to >= nNu
+    if (one) out[gnu.x] = rejected ? __int_as_float(0x7fc00000) : scale * acc.x;
+    if (two) out[gnu.y] = rejected ? __int_as_float(0x7fc00000) : scale * acc.y;
 }
 
 // ---------------------------------------------------------------------------------------

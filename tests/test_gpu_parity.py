@@ -45,11 +45,12 @@ def wl3(torch_cuda):
     return W.make_workload(3, device=_gen_device(torch_cuda))
 
 
-def _run(torch, wl, params, kernel=0, highres=True, models_per_cta=0, nu_order=None):
+def _run(torch, wl, params, kernel=0, highres=True, models_per_cta=0, nu_order=None, fused=False):
     from paper_1910_01070_b200 import Helios
     h = Helios(0)
     if nu_order is not None:
         h.set_nu_order(nu_order)
+    h.set_fused_obs(fused)
     h.setup_workload(wl)
     h.set_kernel(kernel, models_per_cta)
     p = torch.as_tensor(np.ascontiguousarray(params), device="cuda:0")
@@ -528,3 +529,30 @@ def test_wavenumber_order_tables_give_the_same_results(torch_cuda, oracle, wl1, 
         assert np.array_equal(out[0][2], out[1][2]) and np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
     else:
         assert _relerr(out[0][2], out[1][2]) <= 5e-6 and _relerr(out[0][0], out[1][0]) <= 5e-6
+
+
+@pytest.mark.parametrize("kernel", [2, 3], ids=["slab", "levelpar"])
+def test_fused_observation_epilogue(torch_cuda, oracle, wl1, kernel):
+    """HELIOS_OPT_FUSED_OBS: the RT kernel applies convolve + bin in its epilogue with 64-bit integer atomics (no flux
+    buffer).  Against the oracle at the usual tolerances; against the two-kernel path (same flux, the sum over a bin
+    exact in integers instead of fp32: agreement to a few fp32 ulp); bitwise reproducible from run to run and
+    independent of the batch a model is in (integer sums do not depend on the arrival order of the CTAs); rejected
+    models still give NaN spectra and logL = -inf."""
+    params = wl1.params[:40].copy()
+    params[7, 1] = -1.0                                   # f < 0: rejected (R31)
+    ref = oracle.forward_workload(wl1, params=params)
+    ok = np.ones(40, bool); ok[7] = False
+    spec_f, logl_f, _, st = _run(torch_cuda, wl1, params, kernel=kernel, highres=False, fused=True)
+    spec_u, logl_u, _, _ = _run(torch_cuda, wl1, params, kernel=kernel, highres=False, fused=False)
+    assert _relerr(spec_f[ok], ref["spectra"][ok]) <= TOL_FLUX
+    assert np.all(np.isnan(spec_f[7])) and logl_f[7] == -np.inf and st["n_nonfinite"] == 1
+    _check_logl(wl1, logl_f[ok], {"spectra": ref["spectra"][ok], "logl": ref["logl"][ok]}, spec_f[ok])
+    assert _relerr(spec_f[ok], spec_u[ok]) <= 2e-6
+    again = _run(torch_cuda, wl1, params, kernel=kernel, highres=False, fused=True)
+    assert np.array_equal(again[0][ok], spec_f[ok]) and np.array_equal(again[1], logl_f)
+    sub = _run(torch_cuda, wl1, params[8:13], kernel=kernel, highres=False, fused=True)
+    assert np.array_equal(sub[0], spec_f[8:13]) and np.array_equal(sub[1], logl_f[8:13])
+    near = W.near_truth_params(wl1.cfg, 12)
+    refn = oracle.forward_workload(wl1, params=near)
+    _, logln, _, _ = _run(torch_cuda, wl1, near, kernel=kernel, highres=False, fused=True)
+    assert np.max(np.abs(logln - refn["logl"])) <= TOL_LOGL_ABS
