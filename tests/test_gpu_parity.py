@@ -556,3 +556,41 @@ def test_fused_observation_epilogue(torch_cuda, oracle, wl1, kernel):
     refn = oracle.forward_workload(wl1, params=near)
     _, logln, _, _ = _run(torch_cuda, wl1, near, kernel=kernel, highres=False, fused=True)
     assert np.max(np.abs(logln - refn["logl"])) <= TOL_LOGL_ABS
+
+
+def test_measured_peaks_are_plausible(torch_cuda, wl0):
+    """helios_measure_peaks (the roofline denominators of bench.py): the FP32 pipe of an sm_100 SM has 128 lanes and the
+    MUFU unit 16; the micro-benchmarks must land within 10 % below those and never above."""
+    from paper_1910_01070_b200 import Helios
+    h = Helios(0)
+    h.setup_workload(wl0)
+    pk = h.measure_peaks()
+    h.close()
+    assert pk["n_sms"] >= 100 and 500.0 < pk["sm_clock_mhz"] < 3000.0
+    assert 0.9 * 128 <= pk["ffma_per_clk_sm"] <= 128.5 and 0.9 * 128 <= pk["ffma2_per_clk_sm"] <= 128.5
+    assert 0.9 * 16 <= pk["mufu_per_clk_sm"] <= 16.1
+    c1, c2, c3 = pk["ffma2_cycles"]
+    assert 1.9 <= c1 <= c2 <= c3 <= 4.5           # a packed FFMA2 holds the dispatch port >= 2 cycles, more with 3 register pairs
+
+
+def test_stage_timing_mode_gives_the_same_results(torch_cuda, wl1):
+    """HELIOS_OPT_TIMING brackets the kernels with events and launches them without the programmatic-dependent-launch
+    attribute; results must be bit-identical to the default (dependent) launches, and the stage times positive."""
+    import torch
+    from paper_1910_01070_b200 import Helios
+    p = torch.as_tensor(wl1.params[:32], device="cuda:0")
+    out = []
+    for timing in (False, True):
+        h = Helios(0)
+        h.setup_workload(wl1)
+        h.set_timing(timing)
+        spec, logl = h.forward_batch(p)
+        spec2, logl2 = h.forward_batch(p)          # second call: the workspace is reused, nothing may leak from the first
+        torch.cuda.synchronize()
+        assert torch.equal(spec, spec2) and torch.equal(logl, logl2)
+        if timing:
+            st = h.stage_ms()
+            assert st["n_calls"] == 2 and st["prep_ms"] > 0 and st["rt_ms"] > 0 and st["obs_ms"] > 0
+        out.append((spec.cpu().numpy(), logl.cpu().numpy()))
+        h.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
