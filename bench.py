@@ -218,6 +218,7 @@ def run_gpu(args):
     h = Helios(local)
     h.setup_workload(wl)
     h.set_kernel(args.kernel, args.models_per_cta)
+    h.set_fused_obs(args.fused_obs)
     # measured FP32-FMA / MUFU rates of THIS GPU, before the timed region (the roofline denominators)
     try:
         pk = h.measure_peaks()
@@ -344,7 +345,8 @@ def run_gpu(args):
                    "l2": ("opacity table (%.0f MB) fits L2: 256 MiB written between timed steps, only the steps summed"
                           if flush_l2 else "opacity table (%.0f MB) exceeds the 126 MB L2; no flush")
                          % (table_bytes / 1e6),
-                   "kernel": {0: "auto", 1: "direct", 2: "slab", 3: "level-parallel"}[args.kernel]},
+                   "kernel": {0: "auto", 1: "direct", 2: "slab", 3: "level-parallel"}[args.kernel],
+                   "fused_obs": bool(args.fused_obs)},
         "points_per_s": value * cfg.n_nu,
         "stage_ms_per_call": stage,
         "roofline": {"bound": "alu", "kernel": "fused interpolate+tau+RT (k_rt_slab / k_rt_seg)", "achieved": ach_tflops,
@@ -352,7 +354,7 @@ def run_gpu(args):
                                     "useful work per second, not pipe utilisation (ncu pipe counters: profiles/r02_*)",
                      "algorithmic_bytes": must_move_bytes(cfg, B_call),
                      "peak": alu_peak, "unit": "TFLOP/s", "frac": ach_tflops / alu_peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get(cfg.index) if args.batch <= 0 and not teff else None,
+                     "traffic": NCU_TRAFFIC_BYTES.get(cfg.index) if args.batch <= 0 and not teff and not args.fused_obs else None,
                      "peak_source": peak_src, "peak_fma_per_clk_sm": fma_clk, "peak_sm_mhz": sm_mhz,
                      "algorithmic_fma_per_point": fma, "algorithmic_mufu_per_point": mufu,
                      "mufu_frac": ach_mufu / mufu_peak, "mufu_peak_per_clk_sm": pk["mufu_per_clk_sm"],
@@ -398,6 +400,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 direct, 2 slab, 3 level-parallel")
     ap.add_argument("--models-per-cta", type=int, default=0)
+    ap.add_argument("--fused-obs", action="store_true",
+                    help="HELIOS_OPT_FUSED_OBS = 1: convolve + bin in the RT kernel's epilogue, no flux buffer (DESIGN.md section 6)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="override the workload's batch size (sweeps only)")
     args = ap.parse_args()

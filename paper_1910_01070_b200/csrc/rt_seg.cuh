@@ -153,6 +153,8 @@ k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUte
     const int b = blockIdx.x, tile = blockIdx.y;
     if (lane == 0) mbar_init(&bars[warp], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const int inu = tile * kSlabTile + 2 * lane;
+    const int2 gnu = __ldg(reinterpret_cast<const int2*>(a.nu_index + inu));      // static: in flight before the wait
     pdl_wait();                    // records, x and flags come from the prep kernel
     for (int i = threadIdx.x; i < a.x_floats; i += blockDim.x) xs[i] = a.model_x[(size_t)b * a.x_floats + i];
 
@@ -193,8 +195,6 @@ k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUte
     }
     __syncthreads();
 
-    const int inu = tile * kSlabTile + 2 * lane;
-    const int2 gnu = __ldg(reinterpret_cast<const int2*>(a.nu_index + inu));
     const double nu_d0 = a.nu0 + a.dnu * (double)gnu.x, nu_d1 = a.nu0 + a.dnu * (double)gnu.y;
     const float2 nu = make_float2((float)nu_d0, (float)nu_d1);
     const float2 nu_lo = make_float2((float)(nu_d0 - (double)nu.x), (float)(nu_d1 - (double)nu.y));
