@@ -45,7 +45,7 @@ enum {
 #define HELIOS_OPT_KERNEL      1   /* 0 = auto (level-parallel for a handful of models, else staged whenever the table planes fit
                                       shared memory, else direct), 1 = direct (4 taps from global memory; fallback),
                                       2 = staged TMA kernel, 3 = level-parallel kernel (2, 3: error if unavailable) */
-#define HELIOS_OPT_MODELS_PER_CTA 2/* staged kernel: models (= compute warps) per CTA: 8, 16, 24 or 0 = auto */
+#define HELIOS_OPT_MODELS_PER_CTA 2/* staged kernel: models (= compute warps) per CTA: 8, 16, 20, 24, 27 or 0 = auto */
 #define HELIOS_OPT_NU_ORDER    4   /* column order of the resident tables, read by the NEXT helios_load_opacity: 1 (default) =
                                       sorted by a reference opacity, so that the 64 columns a warp owns are optically alike and
                                       take the kernels' warp-uniform thin / thick shortcuts; 0 = wavenumber order.  Results are

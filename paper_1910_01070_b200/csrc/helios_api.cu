@@ -359,8 +359,8 @@ int helios_set_option(helios_ctx* c, int key, int value) {
             if (value < 0 || value > 3) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1, 2 or 3");
             c->opt_kernel = value; return HELIOS_OK;
         case HELIOS_OPT_MODELS_PER_CTA:
-            if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24)
-                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16, 20 or 24");
+            if (value != 0 && value != 8 && value != 16 && value != 20 && value != 24 && value != 27)
+                return fail(c, HELIOS_EINVAL, "HELIOS_OPT_MODELS_PER_CTA must be 0 (auto), 8, 16, 20, 24 or 27");
             c->opt_models_per_cta = value; return HELIOS_OK;
         case HELIOS_OPT_FUSED_OBS:
             c->opt_fused = value ? 1 : 0; return HELIOS_OK;
@@ -717,9 +717,15 @@ static SlabPlan plan_slab(const helios_ctx* c, int B) {
     int nw = c->opt_models_per_cta;
     if (nw == 0) {
         if (B < 16) nw = 8;
-        else {      // padded model slots, weighted by the measured per-model efficiency of the two variants
+        else {      // padded model slots, weighted by the measured per-model efficiency of the variants (27 warps: +1.8 %
+                    // at configs[3] when its groups fill up; its 72-register budget only pays with many angles)
             const double cost24 = (double)((B + 23) / 24 * 24), cost16 = (double)((B + 15) / 16 * 16) / 0.92;
+            const double cost27 = c->A >= 6 ? (double)((B + 26) / 27 * 27) / 1.018 : 1e30;
             nw = cost24 <= cost16 ? 24 : 16;
+            if (cost27 < std::min(cost24, cost16)) {
+                const SlabPlan p27 = slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, 27, c->smem_optin, c->smem_sm);
+                if (p27.ok && p27.ring >= 3) nw = 27;
+            }
         }
     }
     return slab_plan(c->S, c->C, c->nT, c->A, c->S > 0 ? c->n_loads : 0, nw, c->smem_optin, c->smem_sm);

@@ -546,7 +546,7 @@ inline SlabPlan slab_plan(int S, int C, int nT, int A, int n_loads, int want_nw,
     SlabPlan p;
     if (A < 1 || A > kMaxAngles || nT > 256) return p;
     const int nw = want_nw > 0 ? want_nw : 16;
-    if (nw != 8 && nw != 16 && nw != 20 && nw != 24) return p;
+    if (nw != 8 && nw != 16 && nw != 20 && nw != 24 && nw != 27) return p;
     const int target_ctas = nw == 8 ? 3 : 1;
     const size_t plane = sizeof(float) * slab_plane_floats(S, nT);
     const size_t fixed = slab_fixed_bytes(C, nT, nw, slab_x_floats(S, C));
@@ -584,7 +584,7 @@ inline cudaError_t launch_rt_slab_t(const CUtensorMap& tms, const CUtensorMap& t
     return launch_kernel(k_rt_slab<A, NW, MINB>, grid, dim3((NW + 1) * 32), smem, stream, pdl, tms, tmc, a);
 }
 
-struct SlabSmemCache { bool configured[kMaxAngles + 1][4] = {}; };     // [A][models-per-CTA variant], one per context
+struct SlabSmemCache { bool configured[kMaxAngles + 1][5] = {}; };     // [A][models-per-CTA variant], one per context
 
 template <int A>
 inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& tmc, const SlabArgs& a, const SlabPlan& p,
@@ -594,6 +594,7 @@ inline cudaError_t launch_rt_slab_a(const CUtensorMap& tms, const CUtensorMap& t
         case 16: return launch_rt_slab_t<A, 16, 1>(tms, tmc, a, p, cache.configured[A][1], stream, pdl);
         case 20: return launch_rt_slab_t<A, 20, 1>(tms, tmc, a, p, cache.configured[A][2], stream, pdl);
         case 24: return launch_rt_slab_t<A, 24, 1>(tms, tmc, a, p, cache.configured[A][3], stream, pdl);
+        case 27: return launch_rt_slab_t<A, 27, 1>(tms, tmc, a, p, cache.configured[A][4], stream, pdl);
         default: return cudaErrorInvalidValue;
     }
 }
