@@ -34,8 +34,8 @@ NOMINAL_FMA_PER_CLK_SM, NOMINAL_MUFU_PER_CLK_SM, NOMINAL_SM_MHZ = 128.0, 16.0, 1
 HBM_NOMINAL_GBS = 8000.0
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
 # ncu --set full captures summarised in profiles/ (None until captured for this workload).
-NCU_TRAFFIC_BYTES = {2: 220265984 + 8241152,        # profiles/r02_k_rt_slab_cfg2_ncu_full.txt
-                     3: 3726840000 + 2682859000}    # profiles/r02_k_rt_slab_cfg3_ncu_full.txt (flux: scattered 4-byte writes)
+NCU_TRAFFIC_BYTES = {2: 220606720 + 8583680,        # profiles/r02_k_rt_slab_cfg2_ncu_full.txt
+                     3: 3734714000 + 2687789000}    # profiles/r02_k_rt_slab_cfg3_ncu_full.txt (flux: scattered 4-byte writes)
 
 
 def algorithmic_ops(cfg):
