@@ -257,6 +257,7 @@ static void opacity_order(const std::vector<std::vector<float>>& ref_rows, int n
         int best = 0;
         for (int s = 1; s < S; ++s) if (ref_rows[s][i] > ref_rows[best][i]) best = s;
         dom[i] = best; val[i] = ref_rows[best][i];
+        if (!(val[i] == val[i])) val[i] = 0.0f;      // a NaN in the table must not break the ordering of the sort
     }
     std::stable_sort(order.begin(), order.end(), [&](int x, int y) {
         if (dom[x] != dom[y]) return dom[x] < dom[y];
