@@ -255,8 +255,9 @@ def test_batch_invariants(torch_cuda, wl1, kernel):
     assert np.array_equal(spec_r, spec) and np.array_equal(logl_r, logl)
 
 
+@pytest.mark.parametrize("fused", [False, True], ids=["twokernel", "fusedobs"])
 @pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
-def test_ragged_sizes_and_edge_cases(torch_cuda, oracle, kernel):
+def test_ragged_sizes_and_edge_cases(torch_cuda, oracle, kernel, fused):
     """Wavenumber count not a multiple of any tile, odd level count, 1..3 angles,
     single species without CIA, CIA only, bins narrower than a grid cell, no
     instrument profile, clamped temperatures, a non-finite parameter."""
@@ -290,6 +291,7 @@ def test_ragged_sizes_and_edge_cases(torch_cuda, oracle, kernel):
         h.set_atmosphere(L, 100.0, 1e-4, K, A, 2.3, 0.17, 0.5)
         h.set_observation(edges, obs, err, inst)
         h.set_kernel(kernel)
+        h.set_fused_obs(fused)          # the direct kernel ignores it (it always writes the flux)
         p = torch.as_tensor(params, device="cuda:0")
         spec, logl = h.forward_batch(p)
         flux = h.forward_highres(p)
@@ -594,3 +596,38 @@ def test_stage_timing_mode_gives_the_same_results(torch_cuda, wl1):
         out.append((spec.cpu().numpy(), logl.cpu().numpy()))
         h.close()
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+
+
+def test_tall_atmosphere_falls_back_from_the_level_parallel_kernel(torch_cuda, oracle):
+    """More than 8 x 32 + 1 levels: the level-parallel kernel is unavailable (chunks of at most 32 layers), so a small
+    batch on kernel = auto takes the staged kernel; forcing the level-parallel kernel is an error, not a wrong answer."""
+    from paper_1910_01070_b200 import Helios, HeliosError, HELIOS_EINVAL
+    rng = np.random.default_rng(5)
+    nNu, nT, nP, S, C, L, A, K = 300, 6, 5, 2, 1, 300, 2, 3
+    T_grid = np.linspace(200.0, 3200.0, nT); lp_grid = np.linspace(-4.5, 3.0, nP)
+    sigma = (10.0 ** rng.uniform(-26, -22, (S, nT, nP, nNu))).astype(np.float32)
+    cia = (10.0 ** rng.uniform(-9, -7, (C, nT, nNu))).astype(np.float32)
+    nu0, dnu = 3000.0, 2.0
+    edges = np.linspace(nu0, nu0 + dnu * (nNu - 1), 21)
+    inst = np.full(nNu, 6.0)
+    B = 3
+    params = np.column_stack([rng.uniform(4, 5, B), rng.uniform(0.5, 2, B), -np.sort(-rng.uniform(500, 2800, (B, K)), axis=1),
+                              rng.uniform(-7, -3, (B, S))])
+    obs = np.full(20, 1e4); err = np.full(20, 1e3)
+    ref = oracle.forward(T_grid, lp_grid, nu0, dnu, sigma, cia, L, 300.0, 1e-3, K, A, 2.3, 0.17, 1.0, edges, obs, err, inst, params,
+                         want_flux=True)
+    h = Helios(0)
+    h.load_opacity(T_grid, lp_grid, nu0, dnu, sigma, cia)
+    h.set_atmosphere(L, 300.0, 1e-3, K, A, 2.3, 0.17, 1.0)
+    h.set_observation(edges, obs, err, inst)
+    p = torch_cuda.as_tensor(params, device="cuda:0")
+    spec, logl = h.forward_batch(p)
+    flux = h.forward_highres(p)
+    torch_cuda.cuda.synchronize()
+    assert _relerr(flux.cpu().numpy().astype(np.float64), ref["flux_hr"]) <= TOL_FLUX
+    assert _relerr(spec.cpu().numpy().astype(np.float64), ref["spectra"]) <= TOL_FLUX
+    h.set_kernel(3)
+    with pytest.raises(HeliosError) as ei:
+        h.forward_batch(p)
+    assert ei.value.code == HELIOS_EINVAL
+    h.close()
