@@ -163,7 +163,14 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     cfg, name = workload_for(args)
-    wl = workloads.make_workload(cfg.index, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls)
+    # the opacity tables (1.6 GB at configs[3]) are synthesised with torch on the GPU when there is one -- input
+    # preparation, cached under /tmp and never timed; the oracle itself runs on the host cores only
+    try:
+        import torch
+        gen_device = "cuda" if torch.cuda.is_available() else "cpu"
+    except Exception:
+        gen_device = "cpu"
+    wl = workloads.make_workload(cfg.index, batch=cfg.batch if cfg.n_calls == 1 else cfg.batch // cfg.n_calls, device=gen_device)
     import oracle
     cores = oracle.max_threads()
     # keep the whole --steps K --warmup W run within a few minutes: ~60 s of oracle time in total
