@@ -9,7 +9,7 @@
 // level loop is cut into chunks: one CTA = one model x one 64-wavenumber tile, warp c = chunk c
 // of the layers.  Every warp integrates its chunk for an UNKNOWN incoming state, i.e. it carries,
 // per angle, the pair (Psi, C) of  H_out = Psi H_in + C  (H = (I - S)/mu as in rt_slab.cuh; Psi is
-// the chunk's transmission, C its own emission), and one warp then chains the ~15 pairs bottom-up
+// the chunk's transmission, C its own emission), and one warp then chains the 8 pairs bottom-up
 // and forms the flux of Eq. 8-9.  All terms are the ones of the sequential recursion; only the
 // order of the floating-point operations differs.
 //
@@ -31,7 +31,7 @@ namespace helios {
 #define HELIOS_SEG_CHUNKS 8
 #endif
 constexpr int kSegMaxChunks = HELIOS_SEG_CHUNKS;       // warps per CTA
-constexpr int kSegMaxLen = 32;          // layers per chunk (L <= 16 * 32 + 1; longer atmospheres use the staged kernel)
+constexpr int kSegMaxLen = 32;          // layers per chunk (L <= 8 * 32 + 1; longer atmospheres use the staged kernel)
 
 struct SegArgs {
     const float* sigma;       // DEVICE [S][nT][nP][stride]
