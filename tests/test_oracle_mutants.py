@@ -35,6 +35,16 @@ MUTANTS = {
     "M18_density_at_bottom_temperature": ("oracle_number_density(p_bar[l], T[l]), nNu, chi",
                                           "oracle_number_density(p_bar[l], T[0]), nNu, chi", BRUTE),
     "M21_trapezoid_uses_one_level": ("chi + (size_t)(l + 1) * nNu, dz,", "chi + (size_t)(l) * nNu, dz,", BRUTE),
+    # stage functions: one plausible slip each, killed by the closed form that pins the stage
+    "S1_thickness_from_lower_temperature": ("return K_BOLTZMANN * 0.5 * (T_lo + T_hi) /", "return K_BOLTZMANN * 0.5 * (T_lo + T_lo) /",
+                                            "test_total_optical_depth_converges_to_hydrostatic_column"),
+    "S2_flux_without_mu": ("flux += w[k] * mu[k] * I;", "flux += w[k] * I;", "test_rt_isothermal_gives_pi_B"),
+    "S3_gamma_sign_as_printed": ("*gamma = -e - em1 / D;", "*gamma = e - em1 / D;", "test_sc_coefficients_against_eq1_quadrature"),
+    "S4_source_shifted_a_level": ("double dI = beta * S[i] + gamma * S[i - 1];", "double dI = beta * S[i - 1] + gamma * S[i];",
+                                  "test_rt_linear_source_thick_bottom"),
+    "S5_profile_cut_at_4_sigma": ("if (fabs(d) > 5.0 * sg) continue;", "if (fabs(d) > 4.0 * sg) continue;", "test_convolve_closed_forms"),
+    "S6_gravity_as_natural_exponential": ("double g_cgs = pow(10.0, th[0]);", "double g_cgs = exp(th[0]);", BRUTE),
+    "S7_distance_to_the_first_power": ("if (i_d >= 0) scale /= th[i_d] * th[i_d];", "if (i_d >= 0) scale /= th[i_d];", "NEXT:test_whole_path_distance_and_inflation"),
 }
 
 
@@ -47,6 +57,9 @@ def test_mutant_is_killed(name, tmp_path):
         shutil.copytree(os.path.join(ROOT, sub), tmp_path / sub,
                         ignore=shutil.ignore_patterns("*.so", "__pycache__", "test_oracle_mutants.py"))
     (tmp_path / "oracle" / "helios_oracle.c").write_text(src.replace(old, new))
-    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_oracle_pins.py", "-q", "-x", "-k", pin,
+    target = "tests/test_oracle_pins.py"
+    if pin.startswith("NEXT:"):
+        target, pin = "tests/test_oracle_next.py", pin[5:]
+    r = subprocess.run([sys.executable, "-m", "pytest", target, "-q", "-x", "-k", pin,
                         "-p", "no:cacheprovider"], cwd=tmp_path, capture_output=True, text=True, timeout=600)
     assert r.returncode == 1 and "failed" in r.stdout, f"mutant {name} survived {pin}:\n{r.stdout[-1500:]}"
