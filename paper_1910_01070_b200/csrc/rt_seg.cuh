@@ -99,6 +99,29 @@ __device__ __forceinline__ void seg_angles(float2 (&Cc)[A], float2 (&Psi)[A], fl
     }
 }
 
+// General (per-lane) step in the "w form" of rt_slab.cuh: w = 1 - e^{-D} from ex2 (thick lanes) or from the polynomial,
+// w = dtau P_k(dtau) (thin lanes);  C <- C + w (q - C),  Psi <- Psi - w Psi.  dtau is clamped to >= 1e-20 by the caller.
+template <int A, int K0>
+__device__ __forceinline__ void seg_angles_w(float2 (&Cc)[A], float2 (&Psi)[A], float2 dtau, float2 ndtau, float2 q) {
+    if constexpr (K0 < A) {
+        constexpr double mu = kGLmu[A - 1][K0];
+        constexpr float c_exp = (float)(kLog2e / mu), thr = (float)(0.25 * mu);
+        constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
+                        p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
+        const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
+        const float2 wk = __fadd2_rn(bc2(1.0f), neg2(make_float2(ex2_approx(arg.x), ex2_approx(arg.y))));
+        float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
+        P = __ffma2_rn(dtau, P, bc2(p2));
+        P = __ffma2_rn(dtau, P, bc2(p1));
+        P = __ffma2_rn(dtau, P, bc2(p0));
+        const float2 wn = __fmul2_rn(dtau, P);
+        const float2 w = make_float2(dtau.x < thr ? wn.x : wk.x, dtau.y < thr ? wn.y : wk.y);
+        Cc[K0] = __ffma2_rn(w, __fadd2_rn(q, neg2(Cc[K0])), Cc[K0]);
+        Psi[K0] = __ffma2_rn(neg2(w), Psi[K0], Psi[K0]);
+        seg_angles_w<A, K0 + 1>(Cc, Psi, dtau, ndtau, q);
+    }
+}
+
 // The same step when every lane of the warp is on one branch for every angle (LayerLimits of rt_slab.cuh): bitwise the
 // values angle_step_seg selects.
 template <int A, int K0>
@@ -267,7 +290,11 @@ k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUte
             } else {
                 const float2 q = __fmul2_rn(dS, make_float2(rcp_approx(dtau.x), rcp_approx(dtau.y)));
                 if (d_lo >= LayerLimits<A>::all_thick) seg_angles_thick<A, 0>(Cc, Psi, ndtau, q);
-                else seg_angles<A, 0>(Cc, Psi, dtau, ndtau, q, dS);
+                else {
+                    const float2 dtc = make_float2(fmaxf(dtau.x, 1e-20f), fmaxf(dtau.y, 1e-20f));
+                    const float2 qc = __fmul2_rn(dS, make_float2(rcp_approx(dtc.x), rcp_approx(dtc.y)));
+                    seg_angles_w<A, 0>(Cc, Psi, dtc, neg2(dtc), qc);
+                }
             }
         }
         chi_prev = chi; S_prev = Sl;
