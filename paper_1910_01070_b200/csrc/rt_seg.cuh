@@ -69,36 +69,8 @@ __device__ __forceinline__ void mix_half(uint32_t src, const float* x, int S, in
     for (int c = 0; c < C; ++c) gc = __ffma2_rn(bc2(x[S + c]), lds_f2(q + (2 * S + c) * kSlabTile * 4), gc);
 }
 
-// One angle of one layer for the pair (Psi, C).  C takes the step of the sequential recursion (angle_step of
-// rt_slab.cuh: ex2 form for thick lanes, q-free polynomial form for thin ones), Psi the homogeneous part of the
-// same step:  Psi <- e Psi  or  Psi <- Psi - dtau P_k(dtau) Psi.
-template <int A, int K>
-__device__ __forceinline__ void angle_step_seg(float2& Cc, float2& Psi, float2 dtau, float2 ndtau, float2 q, float2 dS) {
-    constexpr double mu = kGLmu[A - 1][K];
-    constexpr float c_exp = (float)(kLog2e / mu), thr = (float)(0.25 * mu);
-    constexpr float p0 = (float)(1.0 / mu), p1 = (float)(kPhiC1 / cpow(mu, 2)), p2 = (float)(kPhiC2 / cpow(mu, 3)),
-                    p3 = (float)(kPhiC3 / cpow(mu, 4)), p4 = (float)(kPhiC4 / cpow(mu, 5));
-    const float2 arg = __fmul2_rn(ndtau, bc2(c_exp));
-    const float2 e = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
-    const float2 bigC = __ffma2_rn(e, Cc, __ffma2_rn(neg2(e), q, q));
-    const float2 bigP = __fmul2_rn(e, Psi);
-    float2 P = __ffma2_rn(dtau, bc2(p4), bc2(p3));
-    P = __ffma2_rn(dtau, P, bc2(p2));
-    P = __ffma2_rn(dtau, P, bc2(p1));
-    P = __ffma2_rn(dtau, P, bc2(p0));
-    const float2 smallC = __ffma2_rn(P, __ffma2_rn(ndtau, Cc, dS), Cc);
-    const float2 smallP = __ffma2_rn(__fmul2_rn(ndtau, P), Psi, Psi);
-    Cc = make_float2(dtau.x < thr ? smallC.x : bigC.x, dtau.y < thr ? smallC.y : bigC.y);
-    Psi = make_float2(dtau.x < thr ? smallP.x : bigP.x, dtau.y < thr ? smallP.y : bigP.y);
-}
-template <int A, int K0>
-__device__ __forceinline__ void seg_angles(float2 (&Cc)[A], float2 (&Psi)[A], float2 dtau, float2 ndtau, float2 q, float2 dS) {
-    if constexpr (K0 < A) {
-        angle_step_seg<A, K0>(Cc[K0], Psi[K0], dtau, ndtau, q, dS);
-        seg_angles<A, K0 + 1>(Cc, Psi, dtau, ndtau, q, dS);
-    }
-}
-
+// One angle of one layer for the pair (Psi, C): C takes the step of the sequential recursion (the thick, thin and
+// general forms of rt_slab.cuh), Psi the homogeneous part of the same step.
 // General (per-lane) step in the "w form" of rt_slab.cuh: w = 1 - e^{-D} from ex2 (thick lanes) or from the polynomial,
 // w = dtau P_k(dtau) (thin lanes);  C <- C + w (q - C),  Psi <- Psi - w Psi.  dtau is clamped to >= 1e-20 by the caller.
 template <int A, int K0>
@@ -122,8 +94,7 @@ __device__ __forceinline__ void seg_angles_w(float2 (&Cc)[A], float2 (&Psi)[A], 
     }
 }
 
-// The same step when every lane of the warp is on one branch for every angle (LayerLimits of rt_slab.cuh): bitwise the
-// values angle_step_seg selects.
+// The same step when every lane of the warp is on one branch for every angle (LayerLimits of rt_slab.cuh).
 template <int A, int K0>
 __device__ __forceinline__ void seg_angles_thick(float2 (&Cc)[A], float2 (&Psi)[A], float2 ndtau, float2 q) {
     if constexpr (K0 < A) {
