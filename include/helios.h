@@ -55,6 +55,10 @@ enum {
                                       write a high-resolution flux: no B x nNu buffer traffic, but the atomics cost more time than the
                                       second kernel they replace (configs[3]: +2.1 ms of 44.5).  0 (default) = the
                                       RT kernel writes the flux, k_obs_apply applies the operator. */
+#define HELIOS_OPT_GRAPHS      6   /* 1 (default) = a helios_forward_batch / helios_loglike_batch call that repeats with the same batch
+                                      size and the same buffers is captured once into a CUDA graph (prep -> RT -> observation) and
+                                      replayed with a single launch from then on (up to 32 distinct calls are kept); 0 = plain launches.
+                                      Only the device-pointer entry points; never under HELIOS_OPT_TIMING. */
 #define HELIOS_OPT_TIMING      3   /* 1 = bracket every stage of the next calls with CUDA events on the context's stream */
 
 typedef struct helios_stats {

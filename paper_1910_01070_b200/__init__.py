@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     helios_get_angles, helios_get_stage_ms, helios_set_tp_elements, helios_set_extras, helios_get_n_params,
     helios_teff_batch, helios_teff_batch_host, helios_measure_peaks, HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD,
     HELIOS_OK, HELIOS_EINVAL, HELIOS_ENOMEM, HELIOS_ECUDA, HELIOS_ESTATE,
-    HELIOS_OPT_KERNEL, HELIOS_OPT_MODELS_PER_CTA, HELIOS_OPT_TIMING, HELIOS_OPT_NU_ORDER, HELIOS_OPT_FUSED_OBS, NU_ORDER_GRID, NU_ORDER_OPACITY,
+    HELIOS_OPT_KERNEL, HELIOS_OPT_MODELS_PER_CTA, HELIOS_OPT_TIMING, HELIOS_OPT_NU_ORDER, HELIOS_OPT_FUSED_OBS, HELIOS_OPT_GRAPHS, NU_ORDER_GRID, NU_ORDER_OPACITY,
     KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB, KERNEL_LEVEL_PARALLEL,
 )
 from .build import build_library, LIB_PATH  # noqa: F401

@@ -23,6 +23,7 @@ HELIOS_OPT_MODELS_PER_CTA = 2
 HELIOS_OPT_TIMING = 3
 HELIOS_OPT_NU_ORDER = 4
 HELIOS_OPT_FUSED_OBS = 5
+HELIOS_OPT_GRAPHS = 6
 NU_ORDER_GRID, NU_ORDER_OPACITY = 0, 1
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB, KERNEL_LEVEL_PARALLEL = 0, 1, 2, 3
 HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD = 1, 2, 4
@@ -357,6 +358,9 @@ class Helios:
     def set_nu_order(self, order: int):
         """Column order of the resident tables for the NEXT load_opacity (NU_ORDER_OPACITY is the default)."""
         helios_set_option(self.ctx, HELIOS_OPT_NU_ORDER, order)
+
+    def set_graphs(self, on: bool):
+        helios_set_option(self.ctx, HELIOS_OPT_GRAPHS, 1 if on else 0)
 
     def set_fused_obs(self, on: bool):
         helios_set_option(self.ctx, HELIOS_OPT_FUSED_OBS, 1 if on else 0)

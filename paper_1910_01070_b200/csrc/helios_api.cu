@@ -63,6 +63,16 @@ struct helios_ctx {
     size_t smem_optin = 0, smem_sm = 0;
     SlabSmemCache slab_smem;
     SegSmemCache seg_smem;
+    // CUDA graphs of whole calls (helios_forward_batch): a call that repeats with the same batch size and buffers is
+    // captured once (prep -> RT -> observation, programmatic dependencies kept) and replayed with one launch
+    struct GraphEntry { int B = 0, P = 0; const void* params = nullptr; const void* spectra = nullptr; const void* logl = nullptr;
+                        cudaGraphExec_t exec = nullptr; unsigned long long last_use = 0; };
+    static constexpr int kGraphEntries = 32;
+    GraphEntry graphs[kGraphEntries];
+    GraphEntry graph_seen;              // the last call that ran without a graph
+    unsigned long long graph_clock = 0;
+    bool graphs_ok = true;              // false after a capture / instantiation failure: plain launches from then on
+    cudaStream_t cap_stream = nullptr;
 
     // ---- observation
     bool have_obs = false, have_data = false;
@@ -84,7 +94,7 @@ struct helios_ctx {
     double* d_params_stage = nullptr; float* d_spectra_stage = nullptr; double* d_logl_stage = nullptr;
 
     // ---- options / statistics
-    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0, opt_nu_order = 1, opt_fused = 0;
+    int opt_kernel = 0, opt_models_per_cta = 0, opt_timing = 0, opt_nu_order = 1, opt_fused = 0, opt_graphs = 1;
     static constexpr int kTimingRing = 64;
     cudaEvent_t ev[kTimingRing][4] = {};
     bool ev_has_obs[kTimingRing] = {};
@@ -126,7 +136,14 @@ static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
     return cudaStreamSynchronize(s);     // src may be a temporary
 }
 
+static void graphs_invalidate(helios_ctx* c) {
+    for (auto& g : c->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); g = helios_ctx::GraphEntry{}; }
+    c->graph_seen = helios_ctx::GraphEntry{};
+}
+
 static void free_all(helios_ctx* c) {
+    graphs_invalidate(c);
+    if (c->cap_stream) { cudaStreamDestroy(c->cap_stream); c->cap_stream = nullptr; }
     dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_Tgrid); dfree(c->d_nu_index);
     dfree(c->d_lvl_p); dfree(c->d_lvl_elem); dfree(c->d_lvl_lw); dfree(c->d_lvl_ip); dfree(c->d_lvl_u);
     dfree(c->d_lvl_pclamp); dfree(c->d_lvl_lnratio);
@@ -348,6 +365,7 @@ void helios_destroy(helios_ctx* c) {
 int helios_set_stream(helios_ctx* c, void* s) {
     if (!c) return HELIOS_EINVAL;
     c->stream = (cudaStream_t)s;
+    graphs_invalidate(c);
     return HELIOS_OK;
 }
 
@@ -355,7 +373,10 @@ const char* helios_last_error(const helios_ctx* c) { return c ? c->err.c_str() :
 
 int helios_set_option(helios_ctx* c, int key, int value) {
     if (!c) return HELIOS_EINVAL;
+    graphs_invalidate(c);
     switch (key) {
+        case HELIOS_OPT_GRAPHS:
+            c->opt_graphs = value ? 1 : 0; return HELIOS_OK;
         case HELIOS_OPT_KERNEL:
             if (value < 0 || value > 3) return fail(c, HELIOS_EINVAL, "HELIOS_OPT_KERNEL must be 0, 1, 2 or 3");
             c->opt_kernel = value; return HELIOS_OK;
@@ -743,6 +764,7 @@ int helios_reserve(helios_ctx* c, int B) {
     dfree(c->d_obs_partial); dfree(c->d_obs_arrived);
     dfree(c->d_params_stage); dfree(c->d_spectra_stage); dfree(c->d_logl_stage); dfree(c->d_addvar);
     dfree(c->d_acc); dfree(c->d_q);
+    graphs_invalidate(c);          // the captured calls point into the old workspace
     c->cap_B = 0;
     const int rf = std::max(direct_rec_floats(c->S, c->C), kSlabRecFloats);
     c->flux_stride = c->stride;
@@ -890,7 +912,7 @@ int helios_forward_highres(helios_ctx* c, int B, int P, const double* params, fl
     return rc;
 }
 
-int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, float* spectra_out, double* logl_out) {
+static int forward_batch_enqueue(helios_ctx* c, int B, int P, const double* params, float* spectra_out, double* logl_out) {
     int rc = check_ready(c, B, P, params, true, logl_out != nullptr);
     if (rc) return rc;
     if (!spectra_out && !logl_out) return fail(c, HELIOS_EINVAL, "both outputs are NULL");
@@ -919,6 +941,62 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     c->n_launches += 1;
     stamp(c, 3);
     if (c->opt_timing) { c->ev_has_obs[c->timed_calls % helios_ctx::kTimingRing] = true; c->timed_calls++; }
+    return HELIOS_OK;
+}
+
+int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, float* spectra_out, double* logl_out) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->opt_graphs || !c->graphs_ok || c->opt_timing) return forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);
+    using Entry = helios_ctx::GraphEntry;
+    auto same = [&](const Entry& g) { return g.B == B && g.P == P && g.params == params && g.spectra == spectra_out && g.logl == logl_out; };
+    ++c->graph_clock;
+    for (auto& g : c->graphs)
+        if (g.exec && same(g)) {                    // replay: one launch for the three kernels
+            CU_TRY(c, cudaSetDevice(c->device));
+            CU_TRY(c, cudaGraphLaunch(g.exec, c->stream));
+            g.last_use = c->graph_clock;
+            c->n_models += B; c->n_launches += 3;
+            return HELIOS_OK;
+        }
+    if (!same(c->graph_seen) || B > c->cap_B) {     // first time: plain launches (this also sizes the workspace and
+        int rc = forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);      // sets the kernels' attributes)
+        if (rc == HELIOS_OK) { c->graph_seen = Entry{}; c->graph_seen.B = B; c->graph_seen.P = P; c->graph_seen.params = params;
+                               c->graph_seen.spectra = spectra_out; c->graph_seen.logl = logl_out; }
+        return rc;
+    }
+    // second time with the same arguments: capture the call on a private stream (the context's stream may be the
+    // legacy default stream, which cannot be captured), instantiate, and launch the graph on the context's stream
+    CU_TRY(c, cudaSetDevice(c->device));
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError(); c->graphs_ok = false;
+        return forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);
+    }
+    cudaStream_t user = c->stream;
+    const unsigned long long models0 = c->n_models, launches0 = c->n_launches;
+    cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
+    int rc = HELIOS_OK;
+    cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed);
+    if (e == cudaSuccess) {
+        c->stream = c->cap_stream;
+        rc = forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);
+        c->stream = user;
+        e = cudaStreamEndCapture(c->cap_stream, &graph);
+    }
+    if (e == cudaSuccess && rc == HELIOS_OK && graph) e = cudaGraphInstantiate(&exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess || rc != HELIOS_OK || !exec) {          // no graphs on this context from now on; run the call plainly
+        cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        c->graphs_ok = false;
+        c->n_models = models0; c->n_launches = launches0;
+        return forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);
+    }
+    Entry* slot = &c->graphs[0];
+    for (auto& g : c->graphs) { if (!g.exec) { slot = &g; break; } if (g.last_use < slot->last_use) slot = &g; }
+    if (slot->exec) cudaGraphExecDestroy(slot->exec);
+    *slot = c->graph_seen; slot->exec = exec; slot->last_use = c->graph_clock;
+    c->graph_seen = Entry{};
+    CU_TRY(c, cudaGraphLaunch(exec, user));                       // the counters were advanced by the captured enqueue
     return HELIOS_OK;
 }
 

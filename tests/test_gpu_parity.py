@@ -631,3 +631,45 @@ def test_tall_atmosphere_falls_back_from_the_level_parallel_kernel(torch_cuda, o
         h.forward_batch(p)
     assert ei.value.code == HELIOS_EINVAL
     h.close()
+
+
+def test_cuda_graph_replay_gives_the_same_results(torch_cuda, oracle, wl1):
+    """HELIOS_OPT_GRAPHS: a call that repeats with the same batch size and buffers is captured on its second
+    occurrence and replayed from the third on.  Replays must be bit-identical to plain launches, follow new
+    parameter VALUES in the same buffer, survive other calls in between, and be dropped when the context changes."""
+    import torch
+    from paper_1910_01070_b200 import Helios
+    pA = torch.as_tensor(wl1.params[:6], device="cuda:0")
+    pB = torch.as_tensor(wl1.params[6:12], device="cuda:0")
+    ref = {}
+    h = Helios(0); h.setup_workload(wl1); h.set_graphs(False)
+    for name, p in (("A", pA), ("B", pB)):
+        s, l = h.forward_batch(p); torch.cuda.synchronize()
+        ref[name] = (s.clone(), l.clone())
+    h.close()
+    h = Helios(0); h.setup_workload(wl1)                       # graphs on (default)
+    h.stats(reset=True)
+    buf = pA.clone()
+    spec = torch.empty((6, h.n_bins), dtype=torch.float32, device="cuda:0")
+    logl = torch.empty((6,), dtype=torch.float64, device="cuda:0")
+    from paper_1910_01070_b200 import helios_forward_batch, helios_loglike_batch
+    for it in range(5):                                        # plain, capture, replay, replay, replay
+        spec.zero_(); logl.zero_()
+        helios_forward_batch(h.ctx, buf, spec, logl); torch.cuda.synchronize()
+        assert torch.equal(spec, ref["A"][0]) and torch.equal(logl, ref["A"][1]), it
+    buf.copy_(pB)                                              # same buffer, new values: the graph reads them at replay
+    helios_forward_batch(h.ctx, buf, spec, logl); torch.cuda.synchronize()
+    assert torch.equal(spec, ref["B"][0]) and torch.equal(logl, ref["B"][1])
+    s2, l2 = h.forward_batch(pA); torch.cuda.synchronize()     # another call (fresh buffers) in between
+    assert torch.equal(s2, ref["A"][0])
+    only = torch.empty((6,), dtype=torch.float64, device="cuda:0")
+    for it in range(3):                                        # logL-only call: its own graph
+        helios_loglike_batch(h.ctx, buf, only); torch.cuda.synchronize()
+        assert torch.equal(only, ref["B"][1])
+    st = h.stats()
+    assert st["n_launches"] == 3 * 10 and st["n_models"] == 6 * 10     # replays are counted like plain calls
+    h.set_observation(wl1.bin_edges, wl1.obs * 1.01, wl1.obs_err, wl1.inst_sigma)     # context changed: graphs dropped
+    for it in range(3):
+        helios_forward_batch(h.ctx, buf, spec, logl); torch.cuda.synchronize()
+        assert torch.equal(spec, ref["B"][0]) and not torch.equal(logl, ref["B"][1])
+    h.close()
