@@ -190,6 +190,29 @@ int helios_forward_batch_host(helios_ctx* ctx, int B, int n_params, const double
 int helios_teff_batch_host(helios_ctx* ctx, int B, int n_params, const double* params_host, double nu_a_cm1,
                            double nu_b_cm1, double* teff_out_host);
 
+/* Step 5 alone (instrument profile, binning, chi-square; Eq. 17, 239, 267-270 Eq. 19), for
+ * callers that must not allocate device memory while they run: a likelihood callback invoked inside a region some
+ * other library is capturing into a CUDA graph, a process whose GPU memory was all handed to a pool at start-up, a
+ * loop that cannot afford the device-wide synchronisation of a cudaFree.  All the other batch entry points size
+ * their workspace with cudaMalloc (helios_reserve); this one calls no cudaMalloc, no cudaFree and no library routine
+ * that allocates.  Its workspace -- the per-model chi-square partial sums and arrival counters of the reduction -- is
+ * a fixed array inside the library image, about 0.5 MB, which every GPU that loads the library holds until the
+ * process ends.
+ *   flux        DEVICE [B][nNu] fp32, rows contiguous: the flux of Eq. 9 on the native grid in wavenumber order, e.g.
+ *               what helios_forward_highres wrote earlier into a buffer the caller owns.
+ *   spectra_out DEVICE [B][n_bins] fp32 or NULL;  logl_out DEVICE [B] fp64 or NULL (needs obs / obs_err).
+ * On the same flux the results are bitwise those of helios_forward_batch.  There are no model flags here: a row of
+ * `flux` that holds NaN/Inf (helios_forward_highres writes NaN for a rejected model) gives NaN bins and logL = -inf.
+ * Limits, fixed by the size of the array: B <= 4096 and B * ceil(n_bins / 8) <= 65536; anything larger returns
+ * HELIOS_EINVAL and enqueues nothing (split the batch).  HELIOS_ESTATE without helios_set_observation, or when
+ * HELIOS_EXTRA_ERROR_INFLATION is on (its variance term comes from the parameter vector, which is not passed here).
+ * The FIRST call on each GPU looks up the array's device address (cudaGetSymbolAddress, which may load the library's
+ * kernels onto that GPU): make that call once during set-up, before any stream capture begins.  Every call, from
+ * every context on that GPU, uses the same array: the counters are cleared on the context's stream at the start of
+ * each call, and two calls that can overlap on the GPU (different streams, different contexts or host threads) race
+ * on it -- keep them on one stream or order them with events.  Enqueues only. */
+int helios_observe_noalloc(helios_ctx* ctx, int B, const float* flux, float* spectra_out, double* logl_out);
+
 /* Copies the counters (synchronises the stream); reset != 0 clears them. */
 int helios_get_stats(helios_ctx* ctx, helios_stats* out, int reset);
 /* Average device time per call of each stage (prep, fused interpolate+RT kernel, fused

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     helios_set_atmosphere, helios_set_observation, helios_reserve, helios_forward_batch,
     helios_loglike_batch, helios_forward_highres, helios_forward_batch_host, helios_get_stats,
     helios_get_angles, helios_get_stage_ms, helios_set_tp_elements, helios_set_extras, helios_get_n_params,
-    helios_teff_batch, helios_teff_batch_host, helios_measure_peaks, HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD,
+    helios_teff_batch, helios_teff_batch_host, helios_measure_peaks, helios_observe_noalloc, HELIOS_EXTRA_DISTANCE, HELIOS_EXTRA_ERROR_INFLATION, HELIOS_EXTRA_GREY_CLOUD,
     HELIOS_OK, HELIOS_EINVAL, HELIOS_ENOMEM, HELIOS_ECUDA, HELIOS_ESTATE,
     HELIOS_OPT_KERNEL, HELIOS_OPT_MODELS_PER_CTA, HELIOS_OPT_TIMING, HELIOS_OPT_NU_ORDER, HELIOS_OPT_FUSED_OBS, HELIOS_OPT_GRAPHS, NU_ORDER_GRID, NU_ORDER_OPACITY,
     KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SLAB, KERNEL_LEVEL_PARALLEL,

@@ -89,12 +89,14 @@ def lib() -> C.CDLL:
         L.helios_teff_batch.argtypes = [_vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
         L.helios_measure_peaks.argtypes = [_vp, C.POINTER(helios_peaks)]
         L.helios_teff_batch_host.argtypes = [_vp, C.c_int, C.c_int, _vp, C.c_double, C.c_double, _vp]
+        L.helios_observe_noalloc.argtypes = [_vp, C.c_int, _vp, _vp, _vp]
         for name in ("helios_create", "helios_set_stream", "helios_set_option", "helios_load_opacity",
                      "helios_set_atmosphere", "helios_set_observation", "helios_reserve",
                      "helios_forward_batch", "helios_loglike_batch", "helios_forward_highres",
                      "helios_forward_batch_host", "helios_get_stats", "helios_get_angles",
                      "helios_get_stage_ms", "helios_set_tp_elements", "helios_set_extras", "helios_get_n_params",
-                     "helios_teff_batch", "helios_measure_peaks", "helios_teff_batch_host"):
+                     "helios_teff_batch", "helios_measure_peaks", "helios_teff_batch_host",
+                     "helios_observe_noalloc"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -249,6 +251,21 @@ def helios_forward_highres(ctx: int, params, flux_out) -> None:
                                              _dev_ptr(flux_out, "float32")))
 
 
+def helios_observe_noalloc(ctx: int, flux, spectra_out=None, logl_out=None) -> None:
+    """Instrument profile + binning + chi-square of a flux the caller already holds, without any device allocation
+    inside the call (include/helios.h: for callers that run under someone else's stream capture, or whose GPU memory is
+    all spoken for).  flux: CUDA float32 [B][n_nu], contiguous; spectra_out: CUDA float32 [B][n_bins] or None;
+    logl_out: CUDA float64 [B] or None.  The outputs are the caller's: this wrapper allocates nothing either.
+    B <= 4096 and B * ceil(n_bins / 8) <= 65536, else HeliosError(HELIOS_EINVAL)."""
+    if flux is None or flux.ndim != 2:
+        raise ValueError("flux must be [B][n_nu]")
+    B = int(flux.shape[0])
+    if spectra_out is not None and (spectra_out.ndim != 2 or spectra_out.shape[0] != B):
+        raise ValueError("spectra_out must be [B][n_bins]")
+    _check(ctx, lib().helios_observe_noalloc(_vp(ctx), B, _dev_ptr(flux, "float32"), _dev_ptr(spectra_out, "float32"),
+                                             _dev_ptr(logl_out, "float64", (B,))))
+
+
 def _host_ptr(a, dtype):
     if a is None:
         return _vp(0)
@@ -401,6 +418,11 @@ class Helios:
 
     def forward_batch_host(self, params_host, spectra_out_host=None, logl_out_host=None):
         helios_forward_batch_host(self.ctx, params_host, spectra_out_host, logl_out_host)
+
+    def observe_noalloc(self, flux, spectra_out=None, logl_out=None):
+        if flux.shape[1] != self.n_nu or (spectra_out is not None and spectra_out.shape[1] != self.n_bins):
+            raise ValueError("flux must be [B][n_nu], spectra_out [B][n_bins]")
+        helios_observe_noalloc(self.ctx, flux, spectra_out, logl_out)
 
     def set_tp_elements(self, n_elements, order, ratio_form=False):
         helios_set_tp_elements(self.ctx, n_elements, order, ratio_form)

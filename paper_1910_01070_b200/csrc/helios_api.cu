@@ -7,6 +7,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1157,3 +1158,145 @@ int helios_get_stats(helios_ctx* c, helios_stats* out, int reset) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// helios_observe_noalloc (include/helios.h): step 5 of the hot path for callers that may not allocate device memory.
+//
+// Who that is: code that runs where cudaMalloc / cudaFree are forbidden or unaffordable -- a sampler callback inside a
+// region another library is capturing into a CUDA graph (an allocation there aborts the capture), a process whose
+// memory pool was handed out in full at start-up (nothing is left for the driver to give), a latency-critical loop
+// that cannot take the device-wide synchronisation a cudaFree implies.  Every other batch entry point of this library
+// grows its workspace through helios_reserve(), i.e. through cudaMalloc.
+//
+// k_obs_apply needs scratch memory beyond its inputs and outputs: one chi-square partial sum per (model, group of 8
+// bins) and one arrival counter per model, used to let the LAST block of a model add the partial sums in a fixed order.
+// The variant below, k_obs_apply_static, is the same kernel with that scratch taken from g_obs_static_scratch, an
+// array that is part of the library image: the CUDA runtime places it in the memory of every GPU the library's
+// module is loaded on, at load time, and it stays there until the process exits (about 0.5 MB per GPU).
+//
+// g_obs_static_scratch is a DEVICE variable.  Inside device code its name is the array.  In host code the same name
+// is only a handle the runtime uses to look the variable up -- it is not the address the GPU sees, and a kernel that
+// was handed it would fault or, on systems where the GPU can reach host memory, quietly work on the wrong bytes.
+// Host code therefore asks the runtime for the device address, once per GPU, with that GPU current
+// (static_scratch_address), and passes that pointer to the kernel.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kStaticMaxBatch = 4096;             // models per call
+constexpr int kStaticMaxGroups = 65536;           // B * ceil(n_bins / 8) per call
+constexpr size_t kStaticPartialBytes = sizeof(double) * (size_t)kStaticMaxGroups;
+constexpr size_t kStaticScratchBytes = kStaticPartialBytes + sizeof(unsigned) * (size_t)kStaticMaxBatch;
+constexpr int kStaticMaxDevices = 64;
+
+static __device__ __align__(256) unsigned char g_obs_static_scratch[kStaticScratchBytes];
+
+static std::mutex g_static_mutex;
+static unsigned char* g_static_ptr[kStaticMaxDevices] = {};     // device address of the array on each GPU, once looked up
+
+// Device address of g_obs_static_scratch on GPU `device`, which must be the current device.  The first call per GPU
+// asks the runtime (this may load the library's module on that GPU, so it should not happen during a stream capture);
+// later calls return the remembered pointer.
+static cudaError_t static_scratch_address(int device, unsigned char** out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[device]) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_obs_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_static_ptr[device] = (unsigned char*)p;
+    }
+    *out = g_static_ptr[device];
+    return cudaSuccess;
+}
+
+// k_obs_apply<8> with its workspace in the static array: one block per (model, 64 bins), a warp owns 8 bins, lanes
+// stride a bin's band of W, shuffle tree, fp64 chi-square term per bin, group sums to `partial`, the block that
+// arrives last at a model adds the groups in the fixed order of k_obs_apply -- so on the same flux the binned
+// spectrum and logL are bitwise those of the allocating path.  Differences: the flux comes from the caller, so there
+// are no model flags (a non-finite flux gives NaN bins and logL = -inf), and the arrival counters are cleared by the
+// host before every launch instead of by the kernel after it.
+__global__ void __launch_bounds__(kObsThreads) k_obs_apply_static(ObsApplyArgs a, unsigned char* scratch) {
+    __shared__ double tree[kObsThreads];
+    __shared__ unsigned ticket;
+    double* partial = reinterpret_cast<double*>(scratch);
+    unsigned* arrived = reinterpret_cast<unsigned*>(scratch + kStaticPartialBytes);
+    const int b = blockIdx.y, chunk = blockIdx.x, n_chunks = gridDim.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const float* F = a.flux + (size_t)b * a.flux_stride;
+    double chi2 = 0.0;
+    const int j0 = chunk * kObsBinsPerCta + warp * 8;
+#pragma unroll 2
+    for (int j = j0; j < min(j0 + 8, a.J); ++j) {
+        const int p0 = a.row_ptr[j], len = a.row_ptr[j + 1] - p0;
+        const float* w = a.W + p0;
+        const float* f = F + a.row_lo[j];
+        float acc0 = 0.0f, acc1 = 0.0f;
+        int i = lane;
+        for (; i + 32 < len; i += 64) {
+            acc0 = fmaf(w[i], f[i], acc0);
+            acc1 = fmaf(w[i + 32], f[i + 32], acc1);
+        }
+        if (i < len) acc0 = fmaf(w[i], f[i], acc0);
+        float acc = acc0 + acc1;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) {
+            if (a.spectra) a.spectra[(size_t)b * a.J + j] = acc;
+            if (a.logl) {
+                const double r = a.obs[j] - (double)acc;
+                chi2 = __dadd_rn(chi2, __dmul_rn(__dmul_rn(r, r), a.inv2var[j]));
+            }
+        }
+    }
+    if (!a.logl) return;
+    const int n_groups = (a.J + 7) / 8;
+    const int g = chunk * (kObsThreads / 32) + warp;
+    if (lane == 0 && g < n_groups) partial[(size_t)b * n_groups + g] = chi2;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        ticket = atomicAdd(&arrived[b], 1u);
+    }
+    __syncthreads();
+    if (ticket != (unsigned)n_chunks - 1) return;
+    __threadfence();
+    double t = 0.0;
+    for (int c = threadIdx.x; c < n_groups; c += kObsThreads) t += __ldcg(&partial[(size_t)b * n_groups + c]);
+    tree[threadIdx.x] = t;
+    __syncthreads();
+#pragma unroll
+    for (int o = kObsThreads / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) tree[threadIdx.x] += tree[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) a.logl[b] = tree[0] == tree[0] ? a.logl_const - tree[0] : -CUDART_INF;
+}
+
+extern "C" int helios_observe_noalloc(helios_ctx* c, int B, const float* flux, float* spectra_out, double* logl_out) {
+    if (!c) return HELIOS_EINVAL;
+    if (!c->have_obs) return fail(c, HELIOS_ESTATE, "observe_noalloc: observation grid not set (helios_set_observation)");
+    if (logl_out && !c->have_data) return fail(c, HELIOS_ESTATE, "observe_noalloc: logL requested but the observation has no data");
+    if (c->extras & HELIOS_EXTRA_ERROR_INFLATION)
+        return fail(c, HELIOS_ESTATE, "observe_noalloc: error inflation takes its variance term from the parameter vector, "
+                    "which this entry point does not see; use helios_forward_batch");
+    if (!flux) return fail(c, HELIOS_EINVAL, "observe_noalloc: flux is NULL");
+    if (!spectra_out && !logl_out) return fail(c, HELIOS_EINVAL, "observe_noalloc: both outputs are NULL");
+    const int n_groups = (c->J + 7) / 8;
+    if (B < 1 || B > kStaticMaxBatch || (long long)B * n_groups > kStaticMaxGroups)
+        return fail(c, HELIOS_EINVAL, "observe_noalloc: batch %d with %d bins exceeds the static scratch array (at most %d models "
+                    "and %d = batch x ceil(n_bins / 8) partial sums per call); split the batch or use helios_forward_batch",
+                    B, c->J, kStaticMaxBatch, kStaticMaxGroups);
+    if (c->device < 0 || c->device >= kStaticMaxDevices)
+        return fail(c, HELIOS_EINVAL, "observe_noalloc: device ordinal %d beyond the %d this entry point keeps an address for",
+                    c->device, kStaticMaxDevices);
+    CU_TRY(c, cudaSetDevice(c->device));
+    unsigned char* scratch = nullptr;
+    CU_TRY(c, static_scratch_address(c->device, &scratch));
+    // the array still holds what the previous call (of any context on this GPU) left: the counters must start at zero;
+    // the partial sums need no clearing, every one a model reads was written by this launch first
+    CU_TRY(c, cudaMemsetAsync(scratch + kStaticPartialBytes, 0, sizeof(unsigned) * (size_t)B, c->stream));
+    ObsApplyArgs oa{};
+    oa.J = c->J; oa.row_ptr = c->d_row_ptr; oa.row_lo = c->d_row_lo; oa.W = c->d_W; oa.flux = flux; oa.flux_stride = c->nNu;
+    oa.obs = c->d_obs; oa.inv2var = c->d_inv2var; oa.logl_const = c->logl_const; oa.spectra = spectra_out; oa.logl = logl_out;
+    k_obs_apply_static<<<dim3((c->J + kObsBinsPerCta - 1) / kObsBinsPerCta, B), kObsThreads, 0, c->stream>>>(oa, scratch);
+    CU_TRY(c, cudaGetLastError());
+    c->n_launches += 1;
+    return HELIOS_OK;
+}
