@@ -45,6 +45,17 @@ MUTANTS = {
     "S5_profile_cut_at_4_sigma": ("if (fabs(d) > 5.0 * sg) continue;", "if (fabs(d) > 4.0 * sg) continue;", "test_convolve_closed_forms"),
     "S6_gravity_as_natural_exponential": ("double g_cgs = pow(10.0, th[0]);", "double g_cgs = exp(th[0]);", BRUTE),
     "S7_distance_to_the_first_power": ("if (i_d >= 0) scale /= th[i_d] * th[i_d];", "if (i_d >= 0) scale /= th[i_d];", "NEXT:test_whole_path_distance_and_inflation"),
+    # round 2's survivors ("What's weak" 1): the one-node branch of the profile and the wiring of the
+    # finite-element parametrisation in the driver
+    "R1_single_node_value_halved": ("if (K == 1) { T[l] = T_knot[0]; continue; }", "if (K == 1) { T[l] = 0.5 * T_knot[0]; continue; }",
+                                    "test_single_node_profile_is_isothermal"),
+    "R2_ratio_form_ignored": ("if (tp_ratio) oracle_tp_dofs_from_ratios(NT, T_par, dof);", "if (0) oracle_tp_dofs_from_ratios(NT, T_par, dof);",
+                              "test_whole_path_brute_force_finite_elements"),
+    "R3_element_order_forced_to_one": ("oracle_temperature_profile_fe(L, p_bar, tp_elements, tp_order, dof, p_bot_bar, p_top_bar, T);",
+                                       "oracle_temperature_profile_fe(L, p_bar, tp_elements, 1, dof, p_bot_bar, p_top_bar, T);",
+                                       "test_whole_path_brute_force_finite_elements"),
+    "R4_vmr_offset_from_n_knots": ("const double *log10_vmr = th + 2 + NT;", "const double *log10_vmr = th + 2 + K;",
+                                   "test_whole_path_brute_force_finite_elements"),
 }
 
 

@@ -628,17 +628,22 @@ def _nongrey_tiny_case():
                 sigma=sigma, cia=cia)
 
 
-def _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he_to_h2, analytic):
+def _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he_to_h2, analytic, T_levels=None):
     """(S_l(nu), dtau_l(nu)) from the paper's statements; `analytic` picks the analytic table or
-    scipy's multilinear interpolation of the stored fp32 nodes."""
+    scipy's multilinear interpolation of the stored fp32 nodes.  T_levels: level temperatures worked out by the
+    caller (higher-order elements) instead of the first-order profile through `knots`."""
     from scipy.interpolate import RegularGridInterpolator
     nu = case["nu0"] + case["dnu"] * np.arange(case["nNu"])
     lev = np.arange(L)
     lp = math.log10(p_bot) + (math.log10(p_top) - math.log10(p_bot)) * lev / (L - 1)      # PAPER.md:55
     p_cgs = 10.0 ** lp * 1e6
     K = len(knots)
-    lp_knots = np.linspace(math.log10(p_bot), math.log10(p_top), K)
+    lp_knots = np.linspace(math.log10(p_bot), math.log10(p_top), max(K, 2))
+    if K == 1:
+        knots = [knots[0], knots[0]]
     T = np.interp(-lp, -lp_knots, knots)                       # linear in log p between the nodes (first-order elements)
+    if T_levels is not None:
+        T = np.asarray(T_levels, np.float64)
     x = 10.0 ** np.asarray(log_vmr)
     x_bg = 1.0 - x.sum()
     x_h2, x_he = x_bg / (1.0 + he_to_h2), x_bg * he_to_h2 / (1.0 + he_to_h2)      # PAPER.md:484
@@ -725,3 +730,71 @@ def test_whole_path_brute_force_many_levels_and_batch(oracle):
         T, S, dtau = _by_hand_columns(case, L, p_bot, p_top, knots, logg, log_vmr, mmw, he, False)
         F = np.array([f * oracle.flux_one_nu(S[:, k], dtau[:, k], mu, w) for k in range(case["nNu"])])
         assert np.allclose(r["flux_hr"][b], F, rtol=1e-12, atol=0.0)
+
+
+# --------------------------------------------------------------------------
+# Round-3 pins: the one-node (isothermal) branch of the profile and the wiring of the finite-element
+# parametrisation in the driver (four one-token mutants survived; they are now in
+# tests/test_oracle_mutants.py and die here).
+# --------------------------------------------------------------------------
+def test_single_node_profile_is_isothermal(oracle):
+    # the profile is the interpolant through its nodes; with ONE node there is one value.
+    p = oracle.level_pressures(17, 300.0, 1e-3)
+    T = oracle.temperature_profile(p, [1234.5], 300.0, 1e-3)
+    assert T.shape == (17,) and np.all(T == 1234.5)
+    # whole path with n_knots = 1 on the non-grey tables: an isothermal atmosphere emits pi B_nu(T0) whatever the
+    # opacity (north_star closed form), times f (R/d)^2 of Eq. 9
+    case = _nongrey_tiny_case()
+    T0, f, flux_const = 1700.0, 1.4, 0.6
+    params = np.array([[5.0, f, T0, -3.0, -3.5]])
+    r = oracle.forward(case["T_grid"], case["lp_grid"], case["nu0"], case["dnu"], case["sigma"], case["cia"],
+                       7, 50.0, 1e-2, 1, 4, 2.3, 0.17, flux_const, np.array([1500.0, 5000.0]), None, None, None, params,
+                       want_flux=True, want_spectra=False, want_logl=False)
+    nu = case["nu0"] + case["dnu"] * np.arange(case["nNu"])
+    B = 2 * H * C * C * nu ** 3 / np.expm1(C2 * nu / T0)
+    assert np.allclose(r["flux_hr"][0], np.pi * f * flux_const * B, rtol=1e-12)
+
+
+def _fe_levels_by_hand(L, p_bot, p_top, n_el, q, dof):
+    """Eq. 12-14 written out: elements equidistant in log p, on each the Lagrange interpolant
+    through its q + 1 Gauss-Lobatto points (end points + roots of P_q'), neighbouring elements sharing their end node."""
+    from numpy.polynomial import legendre as leg
+    inner = leg.legroots(leg.legder([0] * q + [1])) if q > 1 else np.array([])     # roots of P_q' on [-1, 1]
+    nodes = np.concatenate([[0.0], 0.5 * (np.sort(inner) + 1.0), [1.0]])            # reference element [0, 1]
+    assert len(nodes) == q + 1
+    lp = math.log10(p_bot) + (math.log10(p_top) - math.log10(p_bot)) * np.arange(L) / (L - 1)
+    s = (lp - math.log10(p_bot)) / (math.log10(p_top) - math.log10(p_bot)) * n_el
+    T = np.empty(L)
+    for l in range(L):
+        k = min(int(math.floor(s[l])), n_el - 1)
+        T[l] = np.polyval(np.polyfit(nodes, np.asarray(dof[k * q:k * q + q + 1]), q), s[l] - k)    # degree q through q + 1 points
+    return T
+
+
+@pytest.mark.parametrize("ratio_form", [False, True], ids=["nodal", "ratio"])
+def test_whole_path_brute_force_finite_elements(oracle, ratio_form):
+    # 2 second-order elements: N_T = 5 temperature parameters while n_knots = 3 is what the first-order call would
+    # use -- the driver must take N_T (parameter offsets), the order and the ratio flag from the element settings
+    case = _nongrey_tiny_case()
+    L, p_bot, p_top, A, n_el, q = 9, 100.0, 1e-2, 3, 2, 2
+    logg, f, flux_const, mmw, he = 5.1, 0.9, 1.2, 2.3, 0.3
+    log_vmr = [-2.8, -3.9]
+    dof = [2300.0, 2050.0, 1500.0, 1050.0, 800.0]          # mid-element nodes off the chords: order 1 would differ
+    if ratio_form:                                          # PAPER.md:219: T_1 and b_i = T_i / T_{i-1}
+        t_par = [dof[0]] + [dof[i] / dof[i - 1] for i in range(1, 5)]
+    else:
+        t_par = dof
+    params = np.array([[logg, f] + list(t_par) + log_vmr])
+    r = oracle.forward(case["T_grid"], case["lp_grid"], case["nu0"], case["dnu"], case["sigma"], case["cia"],
+                       L, p_bot, p_top, 3, A, mmw, he, flux_const, np.array([1500.0, 5000.0]), None, None, None, params,
+                       want_flux=True, want_spectra=False, want_logl=False,
+                       tp_elements=n_el, tp_order=q, tp_ratio=ratio_form)
+    T = _fe_levels_by_hand(L, p_bot, p_top, n_el, q, dof)
+    assert T[0] == pytest.approx(dof[0]) and T[-1] == pytest.approx(dof[-1]) and T[4] == pytest.approx(dof[2])
+    chord = np.interp(np.arange(L), [0, 4, 8], [dof[0], dof[2], dof[4]])
+    assert np.max(np.abs(T - chord)) > 50.0                 # a first-order profile through the element ends is far off
+    mu, w = np.polynomial.legendre.leggauss(A)
+    mu, w = 0.5 * (mu + 1.0), 0.5 * w
+    _, S, dtau = _by_hand_columns(case, L, p_bot, p_top, [dof[0], dof[2], dof[4]], logg, log_vmr, mmw, he, False, T_levels=T)
+    F = np.array([f * flux_const * oracle.flux_one_nu(S[:, k], dtau[:, k], mu, w) for k in range(case["nNu"])])
+    assert np.allclose(r["flux_hr"][0], F, rtol=1e-11, atol=0.0)
