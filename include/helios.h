@@ -58,7 +58,9 @@ enum {
 #define HELIOS_OPT_GRAPHS      6   /* 1 (default) = a helios_forward_batch / helios_loglike_batch call that repeats with the same batch
                                       size and the same buffers is captured once into a CUDA graph (prep -> RT -> observation) and
                                       replayed with a single launch from then on (up to 32 distinct calls are kept); 0 = plain launches.
-                                      Only the device-pointer entry points; never under HELIOS_OPT_TIMING. */
+                                      Only the device-pointer entry points; never under HELIOS_OPT_TIMING.  Every call that changes
+                                      the context (load_opacity, set_atmosphere, set_tp_elements, set_extras, set_observation,
+                                      set_option, set_stream, a workspace that grows) drops all captured calls. */
 #define HELIOS_OPT_TIMING      3   /* 1 = bracket every stage of the next calls with CUDA events on the context's stream */
 
 typedef struct helios_stats {
@@ -67,6 +69,9 @@ typedef struct helios_stats {
                                           (see helios_forward_batch)                                               */
     unsigned long long n_models;       /* models evaluated since the last reset                                    */
     unsigned long long n_launches;     /* kernels launched by this context since the last reset                    */
+    unsigned long long n_graph_launches; /* calls since the last reset that went out as ONE CUDA-graph launch
+                                          (HELIOS_OPT_GRAPHS) instead of separate kernel launches; their kernels are
+                                          counted in n_launches all the same                                        */
 } helios_stats;
 
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t
@@ -106,7 +111,7 @@ int helios_load_opacity(helios_ctx* ctx, int n_species,
  *   n_knots temperature nodes equidistant in log p (first-order elements);
  *   n_angles Gauss-Legendre angles in mu in (0,1), 1..8;
  *   mean_mol_weight in atomic mass units; he_to_h2 = He/H2 number ratio of the
- *   background gas; flux_const = (R_star/d)^2 of Eq. 9.
+ *   background gas; flux_const = (R_star/d)^2 of Eq. 9, > 0 (HELIOS_EINVAL otherwise).
  * Requires helios_load_opacity() first (the pressure cells are resolved here). */
 int helios_set_atmosphere(helios_ctx* ctx, int n_levels, double p_bottom_bar, double p_top_bar,
                           int n_knots, int n_angles, double mean_mol_weight, double he_to_h2,

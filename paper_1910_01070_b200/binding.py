@@ -41,7 +41,7 @@ class HeliosError(RuntimeError):
 
 class helios_stats(C.Structure):
     _fields_ = [("n_clamped", C.c_ulonglong), ("n_nonfinite", C.c_ulonglong),
-                ("n_models", C.c_ulonglong), ("n_launches", C.c_ulonglong)]
+                ("n_models", C.c_ulonglong), ("n_launches", C.c_ulonglong), ("n_graph_launches", C.c_ulonglong)]
 
 
 class helios_peaks(C.Structure):

@@ -67,11 +67,15 @@ struct helios_ctx {
     // CUDA graphs of whole calls (helios_forward_batch): a call that repeats with the same batch size and buffers is
     // captured once (prep -> RT -> observation, programmatic dependencies kept) and replayed with one launch
     struct GraphEntry { int B = 0, P = 0; const void* params = nullptr; const void* spectra = nullptr; const void* logl = nullptr;
+                        unsigned long long epoch = 0;   // the context's state when the call was seen / captured
                         cudaGraphExec_t exec = nullptr; unsigned long long last_use = 0; };
     static constexpr int kGraphEntries = 32;
     GraphEntry graphs[kGraphEntries];
     GraphEntry graph_seen;              // the last call that ran without a graph
     unsigned long long graph_clock = 0;
+    unsigned long long epoch = 1;       // bumped by every call that changes what the kernels' arguments would be (tables,
+                                        // atmosphere, observation, parametrisation, extras, options, stream, workspace)
+    unsigned long long n_graph_replays = 0;
     bool graphs_ok = true;              // false after a capture / instantiation failure: plain launches from then on
     cudaStream_t cap_stream = nullptr;
 
@@ -137,7 +141,11 @@ static cudaError_t upload(T*& dst, const std::vector<T>& src, cudaStream_t s) {
     return cudaStreamSynchronize(s);     // src may be a temporary
 }
 
+// A captured call holds kernel arguments BY VALUE (device pointers, sizes, logl_const, the tensor maps ...): every
+// setter calls this, so that no graph outlives the state it was captured from; the epoch is a second guard -- an entry
+// whose epoch is not the context's is never replayed, whatever path forgot to come through here.
 static void graphs_invalidate(helios_ctx* c) {
+    ++c->epoch;
     for (auto& g : c->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); g = helios_ctx::GraphEntry{}; }
     c->graph_seen = helios_ctx::GraphEntry{};
 }
@@ -414,6 +422,7 @@ int helios_load_opacity(helios_ctx* c, int S, int nT, const double* T_grid, int 
     for (int k = 0; k < C; ++k) if (!cia[k]) return fail(c, HELIOS_EINVAL, "load_opacity: cia[%d] is NULL", k);
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    graphs_invalidate(c);
     c->have_tables = c->have_atmo = c->have_obs = c->have_data = false;
     dfree(c->d_sigma); dfree(c->d_cia); dfree(c->d_nu_index);
     c->S = S; c->C = C; c->nT = nT; c->nP = nP; c->nNu = nNu; c->nu0 = nu0; c->dnu = dnu;
@@ -513,9 +522,11 @@ int helios_set_atmosphere(helios_ctx* c, int L, double p_bot, double p_top, int 
     if (!(p_bot > p_top) || !(p_top > 0)) return fail(c, HELIOS_EINVAL, "set_atmosphere: need p_bottom > p_top > 0");
     if (K < 1 || K > 64) return fail(c, HELIOS_EINVAL, "set_atmosphere: n_knots %d (1..64)", K);
     if (A < 1 || A > kMaxAngles) return fail(c, HELIOS_EINVAL, "set_atmosphere: n_angles %d (1..%d)", A, kMaxAngles);
-    if (!(mmw > 0) || !(he_to_h2 >= 0) || !std::isfinite(flux_const)) return fail(c, HELIOS_EINVAL, "set_atmosphere: bad mmw / he_to_h2 / flux_const");
+    if (!(mmw > 0) || !(he_to_h2 >= 0) || !(flux_const > 0) || !std::isfinite(flux_const))
+        return fail(c, HELIOS_EINVAL, "set_atmosphere: need mean_mol_weight > 0, he_to_h2 >= 0, flux_const > 0 (finite)");
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    graphs_invalidate(c);
     c->have_atmo = false;
     c->L = L; c->K = K; c->A = A; c->p_bot = p_bot; c->p_top = p_top; c->mmw = mmw; c->he_to_h2 = he_to_h2;
     c->flux_const = flux_const;
@@ -640,6 +651,7 @@ int helios_set_observation(helios_ctx* c, int J, const double* edges, const doub
             return fail(c, HELIOS_EINVAL, "set_observation: inst_sigma[%d] invalid", k);
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    graphs_invalidate(c);
     c->have_obs = c->have_data = false;
     c->J = J;
 
@@ -949,20 +961,23 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     if (!c) return HELIOS_EINVAL;
     if (!c->opt_graphs || !c->graphs_ok || c->opt_timing) return forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);
     using Entry = helios_ctx::GraphEntry;
-    auto same = [&](const Entry& g) { return g.B == B && g.P == P && g.params == params && g.spectra == spectra_out && g.logl == logl_out; };
+    auto same = [&](const Entry& g) { return g.epoch == c->epoch && g.B == B && g.P == P && g.params == params &&
+                                             g.spectra == spectra_out && g.logl == logl_out; };
     ++c->graph_clock;
+    const bool state_ok = c->have_tables && c->have_atmo && c->have_obs && (!logl_out || c->have_data) && B <= c->cap_B;
     for (auto& g : c->graphs)
-        if (g.exec && same(g)) {                    // replay: one launch for the three kernels
+        if (state_ok && g.exec && same(g)) {        // replay: one launch for the three kernels
             CU_TRY(c, cudaSetDevice(c->device));
             CU_TRY(c, cudaGraphLaunch(g.exec, c->stream));
             g.last_use = c->graph_clock;
-            c->n_models += B; c->n_launches += 3;
+            c->n_models += B; c->n_launches += 3; c->n_graph_replays += 1;
             return HELIOS_OK;
         }
     if (!same(c->graph_seen) || B > c->cap_B) {     // first time: plain launches (this also sizes the workspace and
         int rc = forward_batch_enqueue(c, B, P, params, spectra_out, logl_out);      // sets the kernels' attributes)
         if (rc == HELIOS_OK) { c->graph_seen = Entry{}; c->graph_seen.B = B; c->graph_seen.P = P; c->graph_seen.params = params;
-                               c->graph_seen.spectra = spectra_out; c->graph_seen.logl = logl_out; }
+                               c->graph_seen.spectra = spectra_out; c->graph_seen.logl = logl_out;
+                               c->graph_seen.epoch = c->epoch; }      // after the call: helios_reserve may have bumped it
         return rc;
     }
     // second time with the same arguments: capture the call on a private stream (the context's stream may be the
@@ -998,6 +1013,7 @@ int helios_forward_batch(helios_ctx* c, int B, int P, const double* params, floa
     *slot = c->graph_seen; slot->exec = exec; slot->last_use = c->graph_clock;
     c->graph_seen = Entry{};
     CU_TRY(c, cudaGraphLaunch(exec, user));                       // the counters were advanced by the captured enqueue
+    c->n_graph_replays += 1;
     return HELIOS_OK;
 }
 
@@ -1013,6 +1029,7 @@ int helios_set_tp_elements(helios_ctx* c, int n_elements, int order, int ratio_f
         return fail(c, HELIOS_EINVAL, "set_tp_elements: n_elements %d (1..16), order %d (1..4)", n_elements, order);
     CU_TRY(c, cudaSetDevice(c->device));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    graphs_invalidate(c);
     c->tp_order = order; c->tp_ratio = ratio_form ? 1 : 0; c->NT = n_elements * order + 1;
     CU_TRY(c, build_tp(c, n_elements, order));
     c->cap_B = 0;    // the parameter staging buffer depends on P
@@ -1023,6 +1040,7 @@ int helios_set_extras(helios_ctx* c, unsigned flags) {
     if (!c) return HELIOS_EINVAL;
     if (flags & ~(HELIOS_EXTRA_DISTANCE | HELIOS_EXTRA_ERROR_INFLATION | HELIOS_EXTRA_GREY_CLOUD))
         return fail(c, HELIOS_EINVAL, "set_extras: unknown flag in 0x%x", flags);
+    graphs_invalidate(c);
     c->extras = flags;
     c->n_extra = ((flags & HELIOS_EXTRA_DISTANCE) ? 1 : 0) + ((flags & HELIOS_EXTRA_ERROR_INFLATION) ? 1 : 0) +
                  ((flags & HELIOS_EXTRA_GREY_CLOUD) ? 3 : 0);
@@ -1150,9 +1168,10 @@ int helios_get_stats(helios_ctx* c, helios_stats* out, int reset) {
     CU_TRY(c, cudaMemcpyAsync(h, c->d_counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     out->n_clamped = h[0]; out->n_nonfinite = h[1]; out->n_models = c->n_models; out->n_launches = c->n_launches;
+    out->n_graph_launches = c->n_graph_replays;
     if (reset) {
         CU_TRY(c, cudaMemsetAsync(c->d_counters, 0, sizeof h, c->stream));
-        c->n_models = 0; c->n_launches = 0;
+        c->n_models = 0; c->n_launches = 0; c->n_graph_replays = 0;
     }
     return HELIOS_OK;
 }

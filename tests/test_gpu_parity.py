@@ -668,8 +668,94 @@ def test_cuda_graph_replay_gives_the_same_results(torch_cuda, oracle, wl1):
         assert torch.equal(only, ref["B"][1])
     st = h.stats()
     assert st["n_launches"] == 3 * 10 and st["n_models"] == 6 * 10     # replays are counted like plain calls
+    assert st["n_graph_launches"] == 4 + 1 + 2                          # capture + 3 replays, 1 replay, capture + 1 replay
     h.set_observation(wl1.bin_edges, wl1.obs * 1.01, wl1.obs_err, wl1.inst_sigma)     # context changed: graphs dropped
     for it in range(3):
         helios_forward_batch(h.ctx, buf, spec, logl); torch.cuda.synchronize()
         assert torch.equal(spec, ref["B"][0]) and not torch.equal(logl, ref["B"][1])
+    h.close()
+
+
+def test_cuda_graphs_are_dropped_by_every_context_change(torch_cuda, wl1):
+    """A captured call holds its kernels' arguments by value (device pointers, sizes, logl_const, tensor maps).  After
+    EVERY setter the same (buffers, B) call must run the new context, not replay the old graph: each change below is one
+    whose stale replay gives different numbers (a new logl_const, another bin count, another level count, another
+    meaning of the one extra parameter, other tables), the first call after it must not be a graph launch, and the
+    results must equal -- bit for bit -- those of a context that never uses graphs."""
+    import torch
+    import paper_1910_01070_b200 as pkg
+    from paper_1910_01070_b200 import Helios, helios_forward_batch
+    cfg = wl1.cfg
+    B = 6
+    base = np.ascontiguousarray(wl1.params[:B])
+
+    def make(graphs):
+        h = Helios(0); h.setup_workload(wl1); h.set_graphs(graphs)
+        return h
+
+    def run_plain(apply_change, params, n_bins):
+        h = make(False)
+        for ch in apply_change:
+            ch(h)
+        p = torch.as_tensor(params, device="cuda:0")
+        s = torch.empty((B, n_bins), dtype=torch.float32, device="cuda:0")
+        l = torch.empty((B,), dtype=torch.float64, device="cuda:0")
+        helios_forward_batch(h.ctx, p, s, l); torch.cuda.synchronize()
+        h.close()
+        return s, l
+
+    edges2 = np.linspace(wl1.bin_edges[0], wl1.bin_edges[-1], 61)          # 60 bins instead of 120
+    obs2, err2 = np.full(60, float(np.mean(wl1.obs))), np.full(60, float(np.mean(wl1.obs_err)))
+    changes = [
+        # (name, change, parameter block of the calls after it, n_bins after it)
+        ("obs_err (logl_const by value)",
+         lambda h: h.set_observation(wl1.bin_edges, wl1.obs, wl1.obs_err * 1.5, wl1.inst_sigma), base, cfg.n_bins),
+        ("extras: distance", lambda h: h.set_extras(pkg.HELIOS_EXTRA_DISTANCE),
+         np.concatenate([base, np.full((B, 1), 1.7)], axis=1), cfg.n_bins),
+        ("extras: distance -> error inflation, same P", lambda h: h.set_extras(pkg.HELIOS_EXTRA_ERROR_INFLATION),
+         np.concatenate([base, np.full((B, 1), 1.7)], axis=1), cfg.n_bins),
+        ("extras off", lambda h: h.set_extras(0), base, cfg.n_bins),
+        ("n_bins", lambda h: h.set_observation(edges2, obs2, err2, wl1.inst_sigma), base, 60),
+        ("n_levels", lambda h: h.set_atmosphere(cfg.n_levels - 30, cfg.p_bottom_bar, cfg.p_top_bar, cfg.n_knots, cfg.n_angles,
+                                                cfg.mean_mol_weight, cfg.he_to_h2, cfg.flux_const), base, 60),
+        ("tp ratio form, same P", lambda h: h.set_tp_elements(cfg.n_knots - 1, 1, True),
+         np.concatenate([base[:, :3], np.full((B, cfg.n_knots - 1), 0.9), base[:, 2 + cfg.n_knots:]], axis=1), 60),
+        ("tables x 2", lambda h: (h.load_opacity(wl1.T_grid, wl1.log10p_grid, cfg.nu0, cfg.dnu, wl1.sigma * 2.0, wl1.cia),
+                                  h.set_atmosphere(cfg.n_levels, cfg.p_bottom_bar, cfg.p_top_bar, cfg.n_knots, cfg.n_angles,
+                                                   cfg.mean_mol_weight, cfg.he_to_h2, cfg.flux_const),
+                                  h.set_observation(wl1.bin_edges, wl1.obs, wl1.obs_err, wl1.inst_sigma)), base, cfg.n_bins),
+    ]
+    h = make(True)
+    p, s, l = (torch.as_tensor(base, device="cuda:0"), torch.empty((B, cfg.n_bins), dtype=torch.float32, device="cuda:0"),
+               torch.empty((B,), dtype=torch.float64, device="cuda:0"))
+    bufs_first = (p, s, l)
+    for it in range(4):                                        # graphs exist before the first change
+        helios_forward_batch(h.ctx, p, s, l)
+    torch.cuda.synchronize()
+    assert h.stats()["n_graph_launches"] == 3
+    # buffers that stay put over all changes with the same shapes: (params, spectra, logl) keyed by (P, n_bins)
+    bufs = {(base.shape[1], cfg.n_bins): bufs_first}
+    applied = []
+    last = ((base.shape[1], cfg.n_bins), s.clone(), l.clone())
+    for name, change, params, n_bins in changes:
+        key = (params.shape[1], n_bins)
+        if key not in bufs:
+            bufs[key] = (torch.empty((B, params.shape[1]), dtype=torch.float64, device="cuda:0"),
+                         torch.empty((B, n_bins), dtype=torch.float32, device="cuda:0"),
+                         torch.empty((B,), dtype=torch.float64, device="cuda:0"))
+        p, s, l = bufs[key]
+        change(h); applied.append(change)
+        p.copy_(torch.as_tensor(params))
+        ref_s, ref_l = run_plain(applied, params, n_bins)
+        h.stats(reset=True)
+        for it in range(4):                                    # plain, capture, replay, replay: all must give the new context's numbers
+            s.zero_(); l.zero_()
+            helios_forward_batch(h.ctx, p, s, l); torch.cuda.synchronize()
+            if it == 0:
+                assert h.stats()["n_graph_launches"] == 0, name      # the first call after a change is never a graph launch
+            assert torch.equal(s, ref_s) and torch.equal(l, ref_l), (name, it)
+        assert h.stats()["n_graph_launches"] == 3, name
+        if last is not None and last[0] == key:                # same buffers as before the change: the numbers did change
+            assert not (torch.equal(last[1], s) and torch.equal(last[2], l)), name
+        last = (key, s.clone(), l.clone())
     h.close()
