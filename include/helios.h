@@ -44,7 +44,12 @@ enum {
 /* helios_set_option keys */
 #define HELIOS_OPT_KERNEL      1   /* 0 = auto (level-parallel for a handful of models, else staged whenever the table planes fit
                                       shared memory, else direct), 1 = direct (4 taps from global memory; fallback),
-                                      2 = staged TMA kernel, 3 = level-parallel kernel (2, 3: error if unavailable) */
+                                      2 = staged TMA kernel, 3 = level-parallel kernel (2, 3: error if unavailable).
+                                      Reproducibility: each kernel gives a model the same bits whatever batch it is submitted in, but
+                                      the level-parallel kernel composes the layer updates in another floating-point order than the
+                                      staged one (difference <= 5e-6 relative on the flux), and "auto" picks by batch size (B <= 8).
+                                      A sampler that re-evaluates a point in a batch of another size and needs a bitwise-equal logL
+                                      must pin the kernel with 2 or 3. */
 #define HELIOS_OPT_MODELS_PER_CTA 2/* staged kernel: models (= compute warps) per CTA: 8, 16, 20, 24, 27 or 0 = auto */
 #define HELIOS_OPT_NU_ORDER    4   /* column order of the resident tables, read by the NEXT helios_load_opacity: 1 (default) =
                                       sorted by a reference opacity, so that the 64 columns a warp owns are optically alike and

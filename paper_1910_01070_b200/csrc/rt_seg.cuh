@@ -178,13 +178,14 @@ k_rt_seg(const __grid_constant__ CUtensorMap tm_p2, const __grid_constant__ CUte
     // the chunk's first cell, straight from global memory, so that its fetch is in flight while the records are staged
     int first_iT = 0, first_ip = 0;
     if (lane == 0 && n_lev > 0) {
-        first_iT = __float_as_int(__ldg(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats + 9));
+        first_iT = __float_as_int(__ldcg(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats + 9));   // written by k_prep while
+                                               // this grid may already be resident (programmatic launch): not the read-only (.nc) path
         first_ip = __ldg(a.lvl_ip + j0 - 1);
         issue(1, first_iT, first_ip);          // a new cell = two fetches (what 1 here, what 2 in the level loop)
     }
     {
         const float4* src = reinterpret_cast<const float4*>(a.rec + ((size_t)b * a.L + (j0 - 1)) * kSlabRecFloats);
-        for (int i = lane; i < n_lev * (kSlabRecFloats / 4); i += 32) reinterpret_cast<float4*>(rw)[i] = __ldg(src + i);
+        for (int i = lane; i < n_lev * (kSlabRecFloats / 4); i += 32) reinterpret_cast<float4*>(rw)[i] = __ldcg(src + i);
         for (int i = lane; i < n_lev; i += 32) ipw[i] = __ldg(a.lvl_ip + j0 - 1 + i);
     }
     __syncthreads();
@@ -316,7 +317,8 @@ struct SegPlan {
     size_t smem = 0;
 };
 
-// Chunking depends on the number of levels only, so a model's result does not depend on the batch it is in.
+// Chunking depends on the number of levels only, so within THIS kernel a model's result does not depend on the batch it
+// is in.  (Across kernels it does, in the last bits: helios.h, HELIOS_OPT_KERNEL.)
 inline SegPlan seg_plan(int L, int A, int S, int C, int x_floats, size_t smem_optin) {
     SegPlan p;
     if (L < 2 || A < 1 || A > kMaxAngles) return p;

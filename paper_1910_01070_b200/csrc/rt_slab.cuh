@@ -417,7 +417,7 @@ k_rt_slab(const __grid_constant__ CUtensorMap tm_sigma, const __grid_constant__ 
                 const uint32_t ra = rb_a + (uint32_t)(l & (2 * kRecBlkDiv - 1)) * (kSlabRecFloats * 4);
                 r0 = lds_f4(ra); r1 = lds_f4(ra + 16); r2 = lds_f4(ra + 32);
             } else {
-                r0 = __ldg(rp + 3 * l); r1 = __ldg(rp + 3 * l + 1); r2 = __ldg(rp + 3 * l + 2);
+                r0 = __ldcg(rp + 3 * l); r1 = __ldcg(rp + 3 * l + 1); r2 = __ldcg(rp + 3 * l + 2);     // k_prep's output: not .nc under PDL
             }
             const int iT = __float_as_int(r2.y);
             if (fresh || iT != cur_iT) {      // warp-uniform: the model is in another table cell
