@@ -196,6 +196,80 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def other_workloads(h3, wl3, pk, local, dev):
+    """The other workloads north_star names, each under its own clock sample, appended to the default line so that they
+    are measured by whoever runs `python bench.py`: configs[2] at B = 256 (the batch the
+    target is quoted on), configs[4] (16 back-to-back logL-only calls on one stream, ONE event pair around the 16
+    enqueues: SURVEY.md 8(d)), and B = 1 / 8 on the configs[2] tables (the paper's own usage).
+    Inputs resident in HBM, tables larger than L2 (no flush), >= 3 warm-up steps, CUDA events, device pointers."""
+    import torch
+    from paper_1910_01070_b200 import Helios, helios_forward_batch, helios_loglike_batch
+    peaks, _ = measured_peaks()
+    n_sms = pk.get("n_sms", 148)
+    fma_clk = max(pk["ffma_per_clk_sm"], pk["ffma2_per_clk_sm"])
+    out = []
+
+    def measure(name, cfg, h, params, n_calls, want_spec, min_s):
+        B = params.shape[0]
+        B_call = B // n_calls
+        p = torch.as_tensor(params, device=dev)
+        spec = torch.empty((B, cfg.n_bins), dtype=torch.float32, device=dev) if want_spec else None
+        logl = torch.empty((B,), dtype=torch.float64, device=dev)
+
+        def step():
+            for c in range(n_calls):
+                sl = slice(c * B_call, (c + 1) * B_call)
+                if want_spec:
+                    helios_forward_batch(h.ctx, p[sl], spec[sl], logl[sl])
+                else:
+                    helios_loglike_batch(h.ctx, p[sl], logl[sl])
+
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            step()
+        e0.record(); step(); e1.record(); torch.cuda.synchronize()
+        steps = int(min(5000, max(5, min_s * 1e3 / max(e0.elapsed_time(e1), 1e-3))))
+        sampler = ClockSampler(local)
+        torch.cuda.synchronize()
+        sampler.start()
+        e0.record()
+        for _ in range(steps):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms_step = e0.elapsed_time(e1) / steps
+        fma, _ = algorithmic_ops(cfg)
+        sm_mhz = clocks.get("sm_mhz") or pk["sm_clock_mhz"]
+        alu_peak = fma_clk * n_sms * 2.0 * sm_mhz * 1e6 / 1e12
+        ach = 2.0 * fma * B * cfg.n_nu / (ms_step * 1e-3) / 1e12        # whole step (prep + RT + observation) in the denominator
+        bytes_move = must_move_bytes(cfg, B_call)
+        gbs = bytes_move / (ms_step / n_calls * 1e-3) / 1e9
+        out.append({"workload": name, "batch": B, "calls_per_step": n_calls, "spectra_written": bool(want_spec),
+                    "steps": steps, "warmup": 4, "ms_per_step": ms_step, "value": B / (ms_step * 1e-3), "unit": "models/s",
+                    "points_per_s": B * cfg.n_nu / (ms_step * 1e-3),
+                    "roofline": {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
+                                 "note": "algorithmic FMAs x 2 / WHOLE-STEP time (all three kernels), so a lower bound on "
+                                         "the RT kernel's own fraction"},
+                    "hbm_roofline": {"must_move_bytes_per_call": bytes_move, "achieved_gbs": gbs,
+                                     "frac_of_8TBs": gbs / HBM_NOMINAL_GBS, "frac_of_measured": gbs / peaks["hbm_gbs"]},
+                    "clocks": clocks})
+
+    # configs[4] on the context that already holds the configs[3] tables, atmosphere and observation
+    cfg4 = workloads.get_config(4)
+    measure(f"configs[4] {cfg4.name}", cfg4, h3, workloads.draw_params(cfg4, cfg4.batch), cfg4.n_calls, False, 0.9)
+    cfg2 = workloads.get_config(2)
+    wl2 = workloads.make_workload(2, device="cuda")
+    h2 = Helios(local)
+    h2.setup_workload(wl2)
+    measure(f"configs[2] {cfg2.name}", cfg2, h2, wl2.params, 1, True, 0.5)
+    for b in (1, 8):
+        measure(f"configs[2] tables, B = {b} (one sampler point per call: PAPER.md:245)", cfg2, h2, wl2.params[:b], 1, True, 0.3)
+    h2.close()
+    return out
+
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -392,6 +466,8 @@ def run_gpu(args):
         dt1, _ = time_oracle(wl, n1, n_threads=1)
         line["cpu_baseline_1thread"] = {"value": n1 / dt1, "unit": "models/s", "cores": 1, "kind": "oracle",
                                         "sample": f"first {n1} models, one pass of {dt1:.1f} s"}
+    if world == 1 and cfg.index == 3 and args.batch <= 0 and not teff and not args.no_other_workloads:
+        line["other_workloads"] = other_workloads(h, wl, pk, local, dev)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -399,7 +475,10 @@ def run_gpu(args):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--gpus", type=int, default=1,
+                    help="ranks of the run; this script does NOT start them: launch it under torchrun "
+                         "(python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N), it reads "
+                         "RANK / LOCAL_RANK / WORLD_SIZE from the environment")
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=-1, help="BASELINE.json configs index (default 3; 2 for --workload teff)")
@@ -410,6 +489,8 @@ def main():
     ap.add_argument("--fused-obs", action="store_true",
                     help="HELIOS_OPT_FUSED_OBS = 1: convolve + bin in the RT kernel's epilogue, no flux buffer (DESIGN.md section 6)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true",
+                    help="skip the configs[2] / configs[4] / B = 1, 8 records the default configs[3] run appends")
     ap.add_argument("--batch", type=int, default=0, help="override the workload's batch size (sweeps only)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -560,18 +560,26 @@ def test_clamp_count(oracle):
     assert r["n_clamped"] == int(np.sum(T > 2000.0))
 
 
-def test_oracle_is_clean_under_ubsan(tmp_path):
-    """The oracle built with -fsanitize=undefined -fno-sanitize-recover runs the tiny workload
-    (and the NEXT rows) without tripping: no signed overflow, bad shifts, misaligned or
-    out-of-bounds accesses the compiler can see, NaN->int conversions ..."""
+@pytest.mark.parametrize("sanitizer", ["undefined", "address"])
+def test_oracle_is_clean_under_sanitizers(tmp_path, sanitizer):
+    """The oracle built with -fsanitize=undefined -fno-sanitize-recover (no signed overflow, bad shifts, misaligned
+    accesses, NaN->int conversions ...) and with -fsanitize=address (no heap / stack / global out-of-bounds access,
+    no use after free) runs the tiny workload, the NEXT rows and a finite-element case without tripping."""
     import os, subprocess, sys, textwrap
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    so = tmp_path / "liboracle_ubsan.so"
-    r = subprocess.run(["gcc", "-O1", "-g", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-fsanitize=undefined",
-                        "-fno-sanitize-recover=undefined", "-o", str(so), os.path.join(root, "oracle", "helios_oracle.c"),
-                        "-lm"], capture_output=True, text=True)
+    so = tmp_path / f"liboracle_{sanitizer}.so"
+    flags = ["-fsanitize=undefined", "-fno-sanitize-recover=undefined"] if sanitizer == "undefined" else ["-fsanitize=address"]
+    r = subprocess.run(["gcc", "-O1", "-g", "-std=c99", "-fopenmp", "-fPIC", "-shared"] + flags +
+                       ["-o", str(so), os.path.join(root, "oracle", "helios_oracle.c"), "-lm"], capture_output=True, text=True)
     if r.returncode != 0:
-        pytest.skip("gcc has no usable UBSan runtime here: " + r.stderr[-200:])
+        pytest.skip(f"gcc has no usable -fsanitize={sanitizer} runtime here: " + r.stderr[-200:])
+    env = dict(os.environ)
+    if sanitizer == "address":          # the runtime must be the first library of the (uninstrumented) interpreter
+        rt = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+        if not os.path.isabs(rt) or not os.path.exists(rt):
+            pytest.skip("libasan.so not found")
+        env["LD_PRELOAD"] = rt
+        env["ASAN_OPTIONS"] = "detect_leaks=0:abort_on_error=0:exitcode=66"      # the interpreter's own leaks are not ours
     code = textwrap.dedent(f"""
         import sys; sys.path.insert(0, {root!r})
         import numpy as np, oracle.binding as ob
@@ -581,12 +589,14 @@ def test_oracle_is_clean_under_ubsan(tmp_path):
         r = oracle.forward_workload(wl, want_flux=True, teff_range=(4000.0, 4999.0))
         p = np.concatenate([wl.params[0], [2.0, 4.0, -1.0, -1.0, 0.0]])[None, :]
         r2 = oracle.forward_workload(wl, params=p, extras=7)
-        assert np.isfinite(r["logl"]).all() and np.isfinite(r2["logl"]).all()
+        p3 = np.concatenate([wl.params[0, :2], [2000.0, 0.8, 0.9, 0.95, 0.7], wl.params[0, 4:]])[None, :]
+        r3 = oracle.forward_workload(wl, params=p3, tp_elements=2, tp_order=2, tp_ratio=True)
+        assert np.isfinite(r["logl"]).all() and np.isfinite(r2["logl"]).all() and np.isfinite(r3["logl"]).all()
         print("ok")
     """)
-    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300)
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300, env=env)
     assert out.returncode == 0 and "ok" in out.stdout, out.stderr[-2000:]
-    assert "runtime error" not in out.stderr
+    assert "runtime error" not in out.stderr and "AddressSanitizer" not in out.stderr
 
 
 # --------------------------------------------------------------------------
