@@ -12,6 +12,11 @@ pytestmark = pytest.mark.gpu
 
 TOL_FLUX = 1e-4
 TOL_LOGL_ABS = 1e-3
+# all-model logL bound: what a binned-flux error of TOL_FLUX_PROPAGATED * M_j can do to logL.  The measured flux error
+# is 2e-7..5e-7 (fp32 arithmetic; profiles/r03_parity_summary.json) and its terms partly cancel: the measured |dlogL| is
+# <= 0.055 of this bound on every model of every config, a factor ~18.  Rounds 1-2 propagated the full 1e-4 (a factor
+# ~1000, which would not have noticed a 50x regression of the arithmetic).
+TOL_FLUX_PROPAGATED = 2e-6
 
 
 @pytest.fixture(scope="module")
@@ -104,7 +109,7 @@ def _check_logl(wl, logl, ref, spec_gpu=None, tag=None):
     that propagated bound is asserted on every model, and -- tighter -- that the chi-square reduction
     itself is exact: logL equals Eq. 19 evaluated in fp64 on the GPU's own binned spectrum."""
     M = ref["spectra"]
-    e = TOL_FLUX * np.abs(M)
+    e = TOL_FLUX_PROPAGATED * np.abs(M)
     bound = ((np.abs(wl.obs[None, :] - M) * e + 0.5 * e * e) / wl.obs_err[None, :] ** 2).sum(axis=1)
     d = np.abs(logl - ref["logl"])
     assert np.all(d <= bound + TOL_LOGL_ABS), (float(d.max()), float(bound.min()))
@@ -112,13 +117,15 @@ def _check_logl(wl, logl, ref, spec_gpu=None, tag=None):
         own = _logl_from_spectrum(wl, spec_gpu)
         assert np.max(np.abs(logl - own) / np.maximum(1.0, np.abs(own))) <= 1e-9
     _record(tag, max_abs_dlogl=float(d.max()), max_rel_dlogl=float(np.max(d / np.maximum(1.0, np.abs(ref["logl"])))),
-            max_abs_logl=float(np.abs(ref["logl"]).max()), n_models=int(len(d)))
+            max_abs_logl=float(np.abs(ref["logl"]).max()), n_models=int(len(d)),
+            max_dlogl_over_bound=float(np.max(d / (bound + TOL_LOGL_ABS))),
+            **({} if spec_gpu is None else {"max_rel_err_binned_flux": _relerr(spec_gpu, M)}))
     return float(d.max())
 
 
 def _record(tag, **kv):
-    """Measured maxima go to gpurun_out/parity_summary.json (scratch; the numbers quoted in DESIGN.md
-    'logL tolerance' come from it)."""
+    """Measured maxima go to gpurun_out/parity_summary.json (scratch); the copy DESIGN.md 'logL tolerance' quotes is
+    tracked as profiles/r03_parity_summary.json."""
     if tag is None:
         return
     import json, os
@@ -157,8 +164,10 @@ def test_config1_medium_all_models(torch_cuda, oracle, wl1, kernel):
 @pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])
 @pytest.mark.parametrize("cfg_index", [1, 2])
 def test_logl_near_truth_absolute_tolerance(torch_cuda, oracle, wl1, wl2, kernel, cfg_index):
+    """north_star's 1e-3 absolute bound on logL, on three independent near-truth sets of 12 (36 models): round 2 had
+    one set and a 20 % margin at configs[2]; the maximum over the three is what DESIGN.md quotes."""
     wl = {1: wl1, 2: wl2}[cfg_index]
-    params = W.near_truth_params(wl.cfg, 12)
+    params = np.concatenate([W.near_truth_params(wl.cfg, 12, draw=d) for d in range(3)])
     ref = oracle.forward_workload(wl, params=params)
     spec, logl, _, _ = _run(torch_cuda, wl, params, kernel, highres=False)
     assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
@@ -166,7 +175,8 @@ def test_logl_near_truth_absolute_tolerance(torch_cuda, oracle, wl1, wl2, kernel
     assert np.all(red_chi2 < 5.0)                            # the subset really is near the truth
     assert np.max(np.abs(logl - ref["logl"])) <= TOL_LOGL_ABS
     _record(f"configs[{cfg_index}] near truth, kernel {kernel}", max_abs_dlogl=float(np.max(np.abs(logl - ref["logl"]))),
-            max_reduced_chi2=float(red_chi2.max()), n_models=12)
+            max_abs_dlogl_per_draw=[float(np.max(np.abs(logl - ref["logl"])[12 * d:12 * d + 12])) for d in range(3)],
+            max_reduced_chi2=float(red_chi2.max()), n_models=36)
 
 
 def test_config2_full_batch_sampled_models(torch_cuda, oracle, wl2):
@@ -228,7 +238,7 @@ def test_config4_streamed_loglike_only(torch_cuda, oracle, wl3):
 
 
 def test_logl_near_truth_config3(torch_cuda, oracle, wl3):
-    params = W.near_truth_params(wl3.cfg, 4)
+    params = np.concatenate([W.near_truth_params(wl3.cfg, 4, draw=d) for d in range(3)])
     ref = oracle.forward_workload(wl3, params=params)
     spec, logl, _, _ = _run(torch_cuda, wl3, params, 0, highres=False)
     assert _relerr(spec, ref["spectra"]) <= TOL_FLUX
@@ -236,7 +246,22 @@ def test_logl_near_truth_config3(torch_cuda, oracle, wl3):
     assert np.all(red_chi2 < 5.0)
     assert np.max(np.abs(logl - ref["logl"])) <= TOL_LOGL_ABS
     _record("configs[3] near truth", max_abs_dlogl=float(np.max(np.abs(logl - ref["logl"]))),
-            max_reduced_chi2=float(red_chi2.max()), n_models=4)
+            max_reduced_chi2=float(red_chi2.max()), n_models=12)
+    # configs[4]'s call shape: the same vectors inside a 256-model logL-only call (spectra never written), the rest of
+    # the call filled with configs[4]'s own draws; north_star's absolute bound on the near-truth rows
+    from paper_1910_01070_b200 import Helios
+    torch = torch_cuda
+    block = W.draw_params(W.get_config(4))[:256].copy()
+    rows = np.arange(12) * 21 + 3                    # scattered over the call, in several CTAs
+    block[rows] = params
+    h = Helios(0)
+    h.setup_workload(wl3)
+    out = h.loglike_batch(torch.as_tensor(block, device="cuda:0"))
+    torch.cuda.synchronize()
+    h.close()
+    d4 = np.abs(out.cpu().numpy()[rows] - ref["logl"])
+    assert np.max(d4) <= TOL_LOGL_ABS
+    _record("configs[4] near truth (rows of a 256-model logL-only call)", max_abs_dlogl=float(d4.max()), n_models=12)
 
 
 @pytest.mark.parametrize("kernel", [1, 2, 3], ids=["direct", "slab", "levelpar"])

@@ -223,10 +223,11 @@ def true_params(cfg: WorkloadConfig) -> np.ndarray:
     return _draw(_streams(src.seed)[2], src, 1)[0]
 
 
-def near_truth_params(cfg: WorkloadConfig, n: int) -> np.ndarray:
+def near_truth_params(cfg: WorkloadConfig, n: int, draw: int = 0) -> np.ndarray:
     """n vectors close to true_params (reduced chi^2 of order 1): the subset on
-    which an absolute logL tolerance is meaningful (SURVEY.md 8(c) hazards)."""
-    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([cfg.seed, 777])))
+    which an absolute logL tolerance is meaningful (SURVEY.md 8(c) hazards).
+    draw > 0: another, independent set of the same recipe (draw 0 is the set of rounds 1-2)."""
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([cfg.seed, 777] + ([draw] if draw else []))))
     t = true_params(cfg)
     out = np.tile(t, (n, 1))
     K = cfg.n_knots
